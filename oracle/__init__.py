@@ -1,0 +1,207 @@
+"""CPU oracle for the longitudinal tracking hot path -- TEST INFRASTRUCTURE ONLY.
+
+Thin ctypes loader around ``oracle/longtrack_oracle.c`` (read ``longtrack_oracle.h``
+first: scope, citations, pins).  Only ``tests/``, ``__graft_entry__.smoke()`` and the
+``cpu_baseline`` / ``--impl reference`` legs of ``bench.py`` may import this package.
+It imports nothing from ``paper_1610_05801_b200`` and that package imports nothing
+from here.  There is no arithmetic of the method in this file: every number comes out
+of the C functions.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from ctypes import (POINTER, Structure, c_double, c_int, c_size_t, c_ubyte, c_ulonglong,
+                    c_void_p)
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = [os.path.join(_HERE, f) for f in ("longtrack_oracle.c", "map.inc", "longtrack_oracle.h")]
+_LIB = os.path.join(_HERE, "liblongtrack_oracle.so")
+
+EULER_CROMER, LEAPFROG, RUTH4 = 0, 1, 2
+INTEGRATORS = {"euler_cromer": EULER_CROMER, "leapfrog": LEAPFROG, "ruth4": RUTH4}
+
+# gcc flags: plain two-rounding arithmetic (reading G21: no FMA contraction)
+CFLAGS = ["-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra"]
+
+
+class Params(Structure):
+    _fields_ = [("circumference_m", c_double), ("gamma", c_double), ("alpha_c", c_double),
+                ("p0c_eV", c_double), ("charge_e", c_double), ("harmonic", c_int),
+                ("voltage_V", c_double), ("phi_s", c_double), ("ratio2", c_double),
+                ("integrator", c_int)]
+
+
+class Derived(Structure):
+    _fields_ = [(k, c_double) for k in
+                ("R", "beta", "eta", "A", "d", "kappa", "K", "z_max", "H_sep")]
+
+
+class Moments(Structure):
+    _fields_ = [("mean_z", c_double), ("rms_z", c_double), ("mean_d", c_double),
+                ("rms_d", c_double), ("cov_zd", c_double), ("n_in_bucket", c_ulonglong)]
+
+
+MOMENTS_DTYPE = np.dtype([("mean_z", "f8"), ("rms_z", "f8"), ("mean_d", "f8"),
+                          ("rms_d", "f8"), ("cov_zd", "f8"), ("n_in_bucket", "u8")])
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    newest = max(os.path.getmtime(s) for s in _SRC)
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
+        cmd = ["gcc", *CFLAGS, "-o", _LIB, _SRC[0], "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        dp = POINTER(c_double)
+        pp = POINTER(Params)
+        L.lto_derive.argtypes = [pp, POINTER(Derived)]
+        L.lto_derive.restype = c_int
+        L.lto_kick.argtypes = [pp, c_double]
+        L.lto_kick.restype = c_double
+        L.lto_one_turn.argtypes = [pp, dp, dp, c_size_t]
+        L.lto_one_turn.restype = None
+        L.lto_one_turn_ec_adjoint.argtypes = [pp, dp, dp, c_size_t]
+        L.lto_one_turn_ec_adjoint.restype = None
+        L.lto_track.argtypes = [pp, dp, dp, c_size_t, c_ulonglong]
+        L.lto_track.restype = None
+        L.lto_track_ld.argtypes = [pp, c_void_p, c_void_p, c_size_t, c_ulonglong]
+        L.lto_track_ld.restype = None
+        L.lto_track_moments.argtypes = [pp, dp, dp, c_size_t, c_ulonglong, c_void_p]
+        L.lto_track_moments.restype = None
+        L.lto_moments_of.argtypes = [pp, dp, dp, c_size_t, POINTER(Moments)]
+        L.lto_moments_of.restype = None
+        L.lto_hamiltonian.argtypes = [pp, c_double, c_double]
+        L.lto_hamiltonian.restype = c_double
+        L.lto_hamiltonian_n.argtypes = [pp, dp, dp, c_size_t, dp]
+        L.lto_hamiltonian_n.restype = None
+        L.lto_in_bucket.argtypes = [pp, c_double, c_double]
+        L.lto_in_bucket.restype = c_int
+        L.lto_bucket_count.argtypes = [pp, dp, dp, c_size_t]
+        L.lto_bucket_count.restype = c_ulonglong
+        L.lto_bucket_mask.argtypes = [pp, dp, dp, c_size_t, POINTER(c_ubyte)]
+        L.lto_bucket_mask.restype = None
+        L.lto_num_threads.restype = c_int
+        L.lto_set_num_threads.argtypes = [c_int]
+        _lib = L
+    return _lib
+
+
+def make_params(ring: dict, integrator="leapfrog", ratio2: float = 0.0,
+                phi_s: float | None = None) -> Params:
+    """ring: dict with the keys of ``Params`` (see workloads.RING)."""
+    integ = INTEGRATORS[integrator] if isinstance(integrator, str) else int(integrator)
+    return Params(float(ring["circumference_m"]), float(ring["gamma"]),
+                  float(ring["alpha_c"]), float(ring["p0c_eV"]),
+                  float(ring.get("charge_e", 1.0)), int(ring["harmonic"]),
+                  float(ring["voltage_V"]),
+                  float(ring.get("phi_s", 0.0) if phi_s is None else phi_s),
+                  float(ratio2), integ)
+
+
+def _f64(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(POINTER(c_double))
+
+
+def derive(p: Params) -> dict:
+    out = Derived()
+    rc = lib().lto_derive(ctypes.byref(p), ctypes.byref(out))
+    assert rc == 0
+    return {k: getattr(out, k) for k, _ in Derived._fields_}
+
+
+def kick(p: Params, z: float) -> float:
+    return lib().lto_kick(ctypes.byref(p), float(z))
+
+
+def one_turn(p: Params, z, delta):
+    """Returns new (z, delta) arrays after one turn (inputs untouched)."""
+    z, zp = _f64(np.array(z, dtype=np.float64, copy=True).ravel())
+    d, dp_ = _f64(np.array(delta, dtype=np.float64, copy=True).ravel())
+    lib().lto_one_turn(ctypes.byref(p), zp, dp_, z.size)
+    return z, d
+
+
+def one_turn_ec_adjoint(p: Params, z, delta):
+    z, zp = _f64(np.array(z, dtype=np.float64, copy=True).ravel())
+    d, dp_ = _f64(np.array(delta, dtype=np.float64, copy=True).ravel())
+    lib().lto_one_turn_ec_adjoint(ctypes.byref(p), zp, dp_, z.size)
+    return z, d
+
+
+def track(p: Params, z, delta, turns: int):
+    """Returns new (z, delta) arrays after ``turns`` turns (inputs untouched)."""
+    z, zp = _f64(np.array(z, dtype=np.float64, copy=True).ravel())
+    d, dp_ = _f64(np.array(delta, dtype=np.float64, copy=True).ravel())
+    lib().lto_track(ctypes.byref(p), zp, dp_, z.size, int(turns))
+    return z, d
+
+
+def track_ld(p: Params, z, delta, turns: int):
+    """Same map in 80-bit long double; returns np.longdouble arrays."""
+    z = np.ascontiguousarray(np.array(z, dtype=np.longdouble, copy=True).ravel())
+    d = np.ascontiguousarray(np.array(delta, dtype=np.longdouble, copy=True).ravel())
+    assert z.dtype.itemsize == 16, "expects x86-64 80-bit long double padded to 16 bytes"
+    lib().lto_track_ld(ctypes.byref(p), z.ctypes.data, d.ctypes.data, z.size, int(turns))
+    return z, d
+
+
+def track_moments(p: Params, z, delta, turns: int):
+    """Returns (z, delta, moments[turns]); moments[t] = state after turn t+1."""
+    z, zp = _f64(np.array(z, dtype=np.float64, copy=True).ravel())
+    d, dp_ = _f64(np.array(delta, dtype=np.float64, copy=True).ravel())
+    out = np.zeros(int(turns), dtype=MOMENTS_DTYPE)
+    assert out.dtype.itemsize == ctypes.sizeof(Moments)
+    lib().lto_track_moments(ctypes.byref(p), zp, dp_, z.size, int(turns), out.ctypes.data)
+    return z, d, out
+
+
+def moments_of(p: Params, z, delta) -> dict:
+    z, zp = _f64(z)
+    d, dp_ = _f64(delta)
+    out = Moments()
+    lib().lto_moments_of(ctypes.byref(p), zp, dp_, z.size, ctypes.byref(out))
+    return {k: getattr(out, k) for k, _ in Moments._fields_}
+
+
+def hamiltonian(p: Params, z, delta):
+    z, zp = _f64(np.atleast_1d(z))
+    d, dp_ = _f64(np.atleast_1d(delta))
+    H = np.empty_like(z)
+    lib().lto_hamiltonian_n(ctypes.byref(p), zp, dp_, z.size, H.ctypes.data_as(POINTER(c_double)))
+    return H
+
+
+def bucket_count(p: Params, z, delta) -> int:
+    z, zp = _f64(z)
+    d, dp_ = _f64(delta)
+    return int(lib().lto_bucket_count(ctypes.byref(p), zp, dp_, z.size))
+
+
+def bucket_mask(p: Params, z, delta):
+    z, zp = _f64(z)
+    d, dp_ = _f64(delta)
+    m = np.empty(z.size, dtype=np.uint8)
+    lib().lto_bucket_mask(ctypes.byref(p), zp, dp_, z.size, m.ctypes.data_as(POINTER(c_ubyte)))
+    return m.astype(bool)
+
+
+def num_threads() -> int:
+    return int(lib().lto_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().lto_set_num_threads(int(n))

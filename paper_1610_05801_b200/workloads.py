@@ -1,0 +1,136 @@
+"""Seeded synthetic bunches and the five BASELINE.json configurations.
+
+This module is the ONE piece shared by the CUDA path's callers (tests, bench.py) and the
+oracle's callers: it only *generates inputs*.  It holds none of the tracking arithmetic,
+imports neither ``oracle`` nor the CUDA binding, and needs numpy only.
+
+The synthetic bunches stand in for the paper's data files (``data*.csv`` and the
+hollow-bunch beam of PAPER.md:74, :80 -- neither is available, the paper states neither
+their distribution nor the ring settings).  Shapes and sizes follow the paper's runs
+(10^5 x 7*10^4; "usual setting 10^5 to 10^7 macro-particles");
+ring, RF and value distributions follow BASELINE.json:configs[0..4].  Recipe and readings
+(G11, G12, G19): DESIGN.md "Input recipe".
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+
+# BASELINE.json:configs[0]: "C=6911.5 m, R=C/2pi, protons with p0=26 GeV/c and gamma=27.7,
+# alpha_c=1.92e-3, ... h=4620, V=2.0 MV".  gamma and p0 are taken literally and
+# independently (reading G4).
+RING = dict(circumference_m=6911.5, gamma=27.7, alpha_c=1.92e-3, p0c_eV=26.0e9,
+            charge_e=1.0, harmonic=4620, voltage_V=2.0e6, phi_s=0.0)
+
+# BASELINE.json:configs[i]  (seeds: SURVEY.md sec. 8(d))
+CONFIGS = [
+    dict(name="cfg0_tiny_gauss", n=1_000, turns=1_000, integrators=("leapfrog",), ratio2=0.0,
+         dist="gauss", sigma_z=0.23, seed=16100, mode="fused"),
+    dict(name="cfg1_hollow", n=100_000, turns=70_000, integrators=("leapfrog",), ratio2=0.0,
+         dist="hollow", seed=16101, mode="fused"),
+    dict(name="cfg2_large_gauss", n=1_000_000, turns=100_000, integrators=("leapfrog",),
+         ratio2=0.0, dist="gauss", sigma_z=0.35, seed=16102, mode="fused", subsample=10_000),
+    dict(name="cfg3_per_turn_moments", n=10_000_000, turns=1_000, integrators=("leapfrog",),
+         ratio2=0.0, dist="gauss", sigma_z=0.23, seed=16103, mode="per_turn"),
+    dict(name="cfg4_variants", n=1_000_000, turns=10_000,
+         integrators=("euler_cromer", "leapfrog", "ruth4"), ratio2=0.5,
+         dist="gauss", sigma_z=0.30, seed=16104, mode="fused", subsample=100_000),
+]
+
+
+def ring_numbers(ring: dict = RING, ratio2: float = 0.0) -> dict:
+    """Numbers the *input recipe* needs (bucket size, matched momentum spread)."""
+    C = ring["circumference_m"]
+    g = ring["gamma"]
+    h = ring["harmonic"]
+    R = C / (2.0 * math.pi)
+    beta = math.sqrt(1.0 - 1.0 / g ** 2)
+    eta = ring["alpha_c"] - 1.0 / g ** 2
+    A = ring.get("charge_e", 1.0) * ring["voltage_V"] / (beta * ring["p0c_eV"])
+    K = eta * C * A * h / R
+    mu = math.acos(1.0 - 0.5 * K)          # single-harmonic leap-frog tune, always (G19)
+    return dict(R=R, beta=beta, eta=eta, A=A, K=K, mu=mu, Qs=mu / (2.0 * math.pi),
+                kappa=h / R, z_max=math.pi * R / h, H_sep=2.0 * A * R / h,
+                delta_max=2.0 * math.sqrt(A * R / (h * eta * C)), etaC=eta * C, r=ratio2,
+                pot_scale=A * R / h)
+
+
+def matched_sigma_delta(sigma_z: float, ring: dict = RING) -> float:
+    """configs[0]: sigma_delta = sigma_z * 2 pi Q_s / (eta C), Q_s = mu / 2 pi (G19)."""
+    q = ring_numbers(ring)
+    return sigma_z * q["mu"] / q["etaC"]
+
+
+def _inside_separatrix(z, delta, q):
+    """Acceptance test of the input recipe (G11): |z| < z_max and H < H_sep, with the
+    Hamiltonian of the RF actually used (including r)."""
+    ph = q["kappa"] * z
+    pot = (1.0 - np.cos(ph)) + 0.5 * q["r"] * (1.0 - np.cos(2.0 * ph))
+    H = 0.5 * q["etaC"] * delta * delta + q["pot_scale"] * pot
+    return (np.abs(z) < q["z_max"]) & (H < q["H_sep"])
+
+
+def gaussian_bunch(n: int, sigma_z: float, seed: int, ring: dict = RING, ratio2: float = 0.0,
+                   truncate: bool = True):
+    """Gaussian in z and delta (matched sigma_delta), rejection-truncated inside the
+    separatrix.  Draw order (G11): per batch, a block of 2n z values then a block of 2n
+    delta values from ``default_rng(seed)``; keep the first n accepted pairs in draw order."""
+    q = ring_numbers(ring, ratio2)
+    sd = matched_sigma_delta(sigma_z, ring)
+    rng = np.random.default_rng(seed)
+    zs, ds, have = [], [], 0
+    batch = max(2 * n, 16)
+    while have < n:
+        z = rng.normal(0.0, sigma_z, batch)
+        d = rng.normal(0.0, sd, batch)
+        if truncate:
+            m = _inside_separatrix(z, d, q)
+            z, d = z[m], d[m]
+        zs.append(z)
+        ds.append(d)
+        have += z.size
+    z = np.concatenate(zs)[:n].copy()
+    d = np.concatenate(ds)[:n].copy()
+    return z, d
+
+
+def hollow_bunch(n: int, seed: int, ring: dict = RING):
+    """configs[1]: in the normalised plane (z, delta*eta*C/(2 pi Q_s)) the radius is uniform
+    in [0.4, 0.9]*z_max (linear-uniform) and the phase uniform in [0, 2 pi).  Taken literally
+    (G12): no truncation, so part of the ring lies outside the separatrix."""
+    q = ring_numbers(ring)
+    rng = np.random.default_rng(seed)
+    rho = rng.uniform(0.4, 0.9, n) * q["z_max"]
+    theta = rng.uniform(0.0, 2.0 * math.pi, n)
+    z = rho * np.cos(theta)
+    d = rho * np.sin(theta) * q["mu"] / q["etaC"]
+    return z, d
+
+
+def make_bunch(cfg: dict, n: int | None = None, seed: int | None = None, ring: dict = RING):
+    """The bunch of one CONFIGS entry (optionally at another size / seed)."""
+    n = cfg["n"] if n is None else n
+    seed = cfg["seed"] if seed is None else seed
+    if cfg["dist"] == "hollow":
+        return hollow_bunch(n, seed, ring)
+    return gaussian_bunch(n, cfg["sigma_z"], seed, ring, cfg["ratio2"])
+
+
+def subsample_indices(n: int, m: int, seed: int):
+    """Seeded subsample for the oracle (cfg2, cfg4): sorted, without replacement."""
+    return np.sort(np.random.default_rng(seed + 1000).choice(n, m, replace=False))
+
+
+def sigma_delta_for_gate(cfg: dict, ring: dict = RING) -> float:
+    """sigma_delta used to normalise |d delta| in the per-particle gate (G17): the matched
+    value of the config; cfg1 (hollow) uses cfg0's."""
+    return matched_sigma_delta(cfg.get("sigma_z", 0.23), ring)
+
+
+def shard_range(n: int, rank: int, world: int):
+    """Contiguous particle range [lo, hi) of one rank (particles are independent,
+    PAPER.md:163): first n % world ranks get one extra particle."""
+    base, extra = divmod(n, world)
+    lo = rank * base + min(rank, extra)
+    return lo, lo + base + (1 if rank < extra else 0)
