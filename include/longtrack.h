@@ -1,0 +1,225 @@
+/*
+ * longtrack.h -- C ABI of liblongtrack.so: the B200 (sm_100a) hot path of PyHEADTAIL's
+ * longitudinal tracking engine (arxiv/paper_1610_05801, A. Oeftiger, "Parallelisation of
+ * PyHEADTAIL").
+ *
+ * Citations: PAPER.md = the paper's text (/root/reference/PAPER.md when this was written),
+ * BASELINE.json = the task statement at the repo root, DESIGN.md = this repo.
+ *
+ * The operation (sec. 1.1.2): "the particles' motion in longitudinal phase
+ * space -- which comprises two coordinates, the spatial location z and the corresponding
+ * (dimensionless) conjugate momentum delta -- is integrated turn by turn [...] via either
+ * the Euler-Cromer (first order), Leap-Frog (second order Verlet) or Runge-Kutta resp.
+ * Ruth (fourth order) numerical integration algorithms [...] independently done for each
+ * particle's entry in the z and delta arrays".  The paper prints no map equation; the map
+ * is BASELINE.json:configs[0]:
+ *
+ *     one turn (leap-frog):  z -= eta*C/2*delta;  delta += F(z);  z -= eta*C/2*delta
+ *     F(z) = A*[ sin(phi_s + h*z/R) - sin(phi_s) + r*sin(2*h*z/R) ]     (configs[0], [4])
+ *     R = C/2pi, beta = sqrt(1-1/gamma^2), eta = alpha_c - 1/gamma^2, A = q*V/(beta*p0c)
+ *     Euler-Cromer:  delta += F(z);  z -= eta*C*delta                    (G8)
+ *     Ruth4:         three leap-frog steps with factors x1, x0, x1,
+ *                    x1 = 1/(2-2^(1/3)), x0 = -2^(1/3)/(2-2^(1/3))        (G9)
+ *
+ * Loop structure (sec. 2.3): turns are sequential, particles independent;
+ * a thread keeps its particle in registers over many turns ("fused" mode below), or the
+ * turn loop is driven from the host with the state going through device memory every turn
+ * ("per-turn" mode; BASELINE.json:configs[3] adds the per-turn bunch moments).
+ *
+ * Conventions for every call
+ *   - Pointers named *_dev are DEVICE pointers (cudaMalloc / torch CUDA tensors), those
+ *     named *_host are HOST pointers.  The caller owns every array; the library owns the
+ *     tracker handle and a small device scratch (grown lazily, freed by lt_destroy).
+ *   - z and delta are two separate, contiguous arrays of n values (structure of arrays,
+ *     PAPER.md:163-165), updated IN PLACE.  8-byte (fp64) / 4-byte (fp32) alignment is
+ *     required; 16-byte alignment enables the vector path (otherwise a scalar path runs).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
+ *     calls only ENQUEUE work on that stream and return; nothing synchronises the device.
+ *     Results are valid once the caller has synchronised the stream.  The *_host calls are
+ *     the exception: they copy, run and copy back, and return after the data is on the host.
+ *   - Return value: 0 = LT_OK, negative = error (below).  The library never throws, aborts
+ *     or prints.  n == 0 or turns == 0 is LT_OK and a no-op.
+ *   - One tracker may have ONE call in flight at a time (the scratch is per tracker); use
+ *     one tracker per stream for concurrency.  Trackers are cheap.
+ *   - There is no CPU fallback: without a CUDA device every device call returns LT_E_CUDA.
+ */
+#ifndef LONGTRACK_H
+#define LONGTRACK_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LT_VERSION 100 /* 0.1.0 */
+
+typedef struct lt_tracker lt_tracker; /* opaque, library-owned */
+
+typedef enum { LT_EULER_CROMER = 0, LT_LEAPFROG = 1, LT_RUTH4 = 2 } lt_integrator;
+
+enum {
+    LT_OK         = 0,
+    LT_E_NULL     = -1, /* a required pointer is NULL                                     */
+    LT_E_PARAM    = -2, /* gamma <= 1, C <= 0, h <= 0, p0c <= 0, unknown integrator/option,
+                           non-finite parameter, n too large                              */
+    LT_E_UNSTABLE = -3, /* linearised map unstable: K_eff = K*(cos(phi_s)+2r) < 0 or >= 4
+                           (K_eff == 0 is allowed, G10)                         */
+    LT_E_ALIGN    = -4, /* array pointer not aligned to its element size                  */
+    LT_E_CUDA     = -5, /* a CUDA runtime call failed; see lt_last_cuda_error()           */
+    LT_E_NOMEM    = -6  /* host allocation failed                                         */
+};
+
+/* Ring / RF parameters: BASELINE.json:north_star (1) "(C, gamma, alpha_c, h, V, phi_s,
+ * integrator)" plus p0 and the charge that A needs (configs[0]) and the second-harmonic
+ * amplitude ratio (configs[4]). */
+typedef struct {
+    double circumference_m; /* C [m]                                             */
+    double gamma;           /* Lorentz gamma (> 1); beta is derived from it       */
+    double alpha_c;         /* momentum compaction factor                         */
+    double p0c_eV;          /* reference momentum times c [eV]                    */
+    double charge_e;        /* q in units of e (1 for protons)                    */
+    int    harmonic;        /* h (> 0)                                            */
+    double voltage_V;       /* V [volt]                                           */
+    double phi_s;           /* synchronous phase [rad]; 0 in every BASELINE config */
+    double ratio2;          /* r: amplitude ratio of the harmonic at 2h; 0 = off   */
+    int    integrator;      /* lt_integrator                                      */
+} lt_params;
+
+/* Derived constants (notation of DESIGN.md): filled by lt_derived(). */
+typedef struct {
+    double R;      /* C/(2 pi)                                                   */
+    double beta;   /* sqrt(1 - 1/gamma^2)                                        */
+    double eta;    /* alpha_c - 1/gamma^2                                        */
+    double A;      /* q V / (beta p0c)                                           */
+    double d;      /* eta C / 2                                                  */
+    double kappa;  /* h / R                                                      */
+    double K;      /* eta C A h / R  (single-harmonic, phi_s = 0)                */
+    double mu;     /* arccos(1 - K/2): exact leap-frog / Euler-Cromer tune [rad] */
+    double z_max;  /* pi R / h                                                   */
+    double H_sep;  /* 2 A R / h                                                  */
+} lt_derived_t;
+
+/* Bunch moments of one state (BASELINE.json:configs[3]: "per-turn mean and rms of z and
+ * delta"): population rms about the mean over all n particles (G14), the z-delta
+ * covariance, and the bucket-membership count of the same state (north_star). */
+typedef struct {
+    double mean_z, rms_z, mean_d, rms_d, cov_zd;
+    unsigned long long n_in_bucket;
+} lt_moments;
+
+/* Raw sums behind lt_moments; additive over disjoint particle ranges, which is what a
+ * multi-GPU run all-reduces. */
+typedef struct {
+    double n;                       /* particle count (as double so one SUM all-reduce does it) */
+    double sum_z, sum_zz, sum_d, sum_dd, sum_zd;
+    double n_in_bucket;             /* exact for counts < 2^53 */
+    double pad_;                    /* keeps sizeof == 64 */
+} lt_sums;
+
+/* Options for lt_set_option / lt_get_option. */
+enum {
+    LT_OPT_SPLIT_DRIFTS   = 1, /* 0 (default): fused mode merges the trailing half drift of a
+                                  turn with the leading one of the next (one FMA with 2d);
+                                  1: every half drift is its own FMA, bit-identical to the
+                                  per-turn kernel and to any chunking by the caller.       */
+    LT_OPT_CHUNK_TURNS    = 2, /* turns per fused kernel launch (default 2^22); the result
+                                  of one call does not depend on it     */
+    LT_OPT_FUSED_ILP      = 3, /* particles per thread in fused mode: 0 = planner decides  */
+    LT_OPT_FUSED_BLOCK    = 4, /* threads per block in fused mode: 0 = planner decides     */
+    LT_OPT_PER_TURN_GRAPH = 5, /* 1 (default): per-turn launches are replayed from a CUDA
+                                  graph in batches; 0: plain stream launches               */
+    LT_OPT_PER_TURN_CTAS_PER_SM = 6, /* persistent CTAs per SM of the per-turn kernel      */
+    LT_OPT_PER_TURN_REVERSE = 7, /* 1 (default): odd turns walk the arrays backwards so the
+                                  tail the previous turn left in L2 is read first          */
+    LT_OPT_FUSED_MODE     = 8, /* 0 (default): planner picks the persistent kernel in static or
+                                  dynamic form; 1: plain one-thread-per-particle kernel
+                                  (LT_OPT_FUSED_ILP / _BLOCK apply); 3: force dynamic        */
+    LT_OPT_ITEM_TURNS     = 9, /* turns per work item of the dynamic persistent kernel
+                                  (0 = planner: 256..1024); results do not depend on it            */
+    LT_OPT_WARPS_PER_SMSP = 10,/* resident warps per SM sub-partition of the persistent kernel
+                                  (0 = planner; 1..8, or even values up to 16)              */
+    LT_OPT_FLIP_ON_Q      = 11 /* where the sign of the reduced sine is applied: -1 planner,
+                                  0 on the argument, 1 on the polynomial; same bits either way */
+};
+
+/* Counters for lt_get_stat. */
+enum {
+    LT_STAT_KERNEL_LAUNCHES = 1, /* kernels launched by this tracker since creation        */
+    LT_STAT_LAST_GRID       = 2, /* grid / block / ilp of the last fused launch            */
+    LT_STAT_LAST_BLOCK      = 3,
+    LT_STAT_LAST_ILP        = 4,
+    LT_STAT_SM_COUNT        = 5,
+    LT_STAT_LAST_MODE       = 6, /* 1 plain, 2 persistent static, 3 persistent dynamic          */
+    LT_STAT_LAST_ITEM_TURNS = 7
+};
+
+/* -- lifetime ------------------------------------------------------------------------ */
+
+/* Validates p, derives the constants, allocates the handle.  Touches no GPU. */
+int lt_create(const lt_params *p, lt_tracker **out);
+int lt_destroy(lt_tracker *tr); /* frees the handle and its device scratch; NULL is LT_OK */
+int lt_derived(const lt_tracker *tr, lt_derived_t *out);
+int lt_set_option(lt_tracker *tr, int option, long long value);
+int lt_get_option(const lt_tracker *tr, int option, long long *value);
+int lt_get_stat(const lt_tracker *tr, int stat, long long *value);
+const char *lt_strerror(int code);
+int lt_last_cuda_error(const lt_tracker *tr); /* cudaError_t of the last LT_E_CUDA, else 0 */
+int lt_version(void);
+
+/* -- fused multi-turn mode ("a single thread contains a long enough loop to
+ *    make use of the registers [...] and circumvent memory access") ------------------------
+ * Advances every particle by `turns` turns.  z/delta are read once at entry and written once
+ * at exit of each chunk (LT_OPT_CHUNK_TURNS); FP64-pipe bound. */
+int lt_track_fused(lt_tracker *tr, double *z_dev, double *delta_dev, size_t n,
+                   unsigned long long turns, void *stream);
+int lt_track_fused_f32(lt_tracker *tr, float *z_dev, float *delta_dev, size_t n,
+                       unsigned long long turns, void *stream);
+
+/* -- per-turn mode ("each GPU thread advances the corresponding particle by one
+ *    turn"; BASELINE.json:configs[3]) -----------------------------------------------------
+ * One kernel launch per turn; each reads and writes z/delta (32 B per particle-turn in fp64)
+ * and reduces the turn's moments in the same pass.  moments_dev / sums_dev: [turns] entries
+ * or NULL; entry t describes the state AFTER turn t+1.  In the fp32 variant the state is
+ * fp32 and the sums are accumulated in fp64.  HBM-bandwidth bound. */
+int lt_track_per_turn(lt_tracker *tr, double *z_dev, double *delta_dev, size_t n,
+                      unsigned long long turns, lt_moments *moments_dev, lt_sums *sums_dev,
+                      void *stream);
+int lt_track_per_turn_f32(lt_tracker *tr, float *z_dev, float *delta_dev, size_t n,
+                          unsigned long long turns, lt_moments *moments_dev,
+                          lt_sums *sums_dev, void *stream);
+
+/* -- observables of the current state ---------------------------------------------------- */
+
+/* Bucket membership (BASELINE.json:north_star "bucket-membership counts (exact)";
+ * DESIGN.md G15): count_dev[0] = #{ i : |z_i| < z_max  and  H(z_i, delta_i) < H_sep }. */
+int lt_bucket_count(lt_tracker *tr, const double *z_dev, const double *delta_dev, size_t n,
+                    unsigned long long *count_dev, void *stream);
+int lt_bucket_count_f32(lt_tracker *tr, const float *z_dev, const float *delta_dev, size_t n,
+                        unsigned long long *count_dev, void *stream);
+/* Moments of the current state (no tracking); either output may be NULL. */
+int lt_moments_now(lt_tracker *tr, const double *z_dev, const double *delta_dev, size_t n,
+                   lt_moments *moments_dev, lt_sums *sums_dev, void *stream);
+
+/* Host helper: turns `count` raw sums (e.g. after an all-reduce over ranks) into moments. */
+int lt_moments_from_sums(const lt_sums *sums_host, size_t count, lt_moments *out_host);
+
+/* -- host-buffer entry point (the paper's long_tracking_cu flow, PAPER.md:242-260:
+ *    cudaMalloc, cudaMemcpyHostToDevice, kernel, cudaMemcpyDeviceToHost) ------------------
+ * z_host/delta_host: n doubles each (pinned memory makes the copies asynchronous but is not
+ * required).  Uses an internal stream and staging buffers kept by the tracker; returns after
+ * the results are in the host arrays.  count_host may be NULL; if not, it receives the
+ * bucket-membership count of the final state. */
+int lt_track_fused_host(lt_tracker *tr, double *z_host, double *delta_host, size_t n,
+                        unsigned long long turns, unsigned long long *count_host);
+
+/* -- roofline probes (measurement only, not on the hot path) ------------------------------
+ * Runs a dependent-chain DFMA kernel (`chains` independent chains per thread, `iters` FMAs
+ * per chain) and returns achieved FP64 lane-instructions per second in *rate. Synchronises. */
+int lt_probe_fp64(int blocks, int threads, int chains, long long iters, double *rate_host,
+                  double *ms_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LONGTRACK_H */

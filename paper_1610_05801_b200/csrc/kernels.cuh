@@ -1,0 +1,609 @@
+// kernels.cuh -- sm_100a device code of liblongtrack (CUDA path only; shares nothing with oracle/).
+//
+// Notation: the state of a particle is (z, delta).  Inside the kernels the position
+// is carried as the RF phase in HALF PERIODS,  v = kappa*z/pi  (kappa = h/R), so that
+//     sin(kappa z) = sin(pi v) = (-1)^n sin(pi f),   n = rint(v),  f = v - n  in [-1/2, 1/2]
+// and the range reduction is EXACT for any |v| < 2^51 (unbound particles stream to |v| ~ 1e4):
+//     t = v + 1.5*2^52  (DADD; the low mantissa bit of t is the parity of n)
+//     n = t - 1.5*2^52  (DADD, exact)        f = v - n  (DADD, exact)
+// The sign (-1)^n is XORed into the sign bit of f on the integer pipe; sin(pi f) = f*S(f^2) is
+// a degree-7 polynomial in s = f^2 with the kick amplitude folded into its coefficients, so
+//     delta += A sin(kappa z)   ==   delta = fma(f_signed, S_A(s), delta).
+// FP64-pipe instructions per particle-turn, leap-frog / Euler-Cromer, single harmonic, merged
+// drifts:  1 (drift) + 3 (reduction) + 1 (s) + 7 (Horner) + 1 (kick FMA) = 13.
+// (BASELINE.json:configs[0] gives the map; PAPER.md:175 the register-resident turn loop.)
+#pragma once
+
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace lt {
+
+#ifndef LT_TURN_UNROLL
+#define LT_TURN_UNROLL 16
+#endif
+
+constexpr int kEulerCromer = 0, kLeapfrog = 1, kRuth4 = 2;
+constexpr int kMaxSin = 8, kMaxCos = 9;
+
+// ------------------------------------------------------------------------------------------
+// Per-tracker constants, passed by value as a __grid_constant__ kernel parameter: they sit in
+// the constant bank and feed DFMA/FFMA as direct operands (no registers, no loads).
+// ------------------------------------------------------------------------------------------
+template <typename T>
+struct MapConsts {
+    T to_phase;             // kappa/pi:        v = z * to_phase
+    T from_phase;           // pi/kappa:        z = v * from_phase
+    T d;                    // eta*C/2          (half-turn drift of z, exact path)
+    T c_half;               // d*kappa/pi       (half-turn drift of v)
+    // drift coefficients of v per stage, fast path.  Leap-frog: lead = c_half, mid unused,
+    // trail = c_half, merged = 2 c_half.  Ruth4: lead = x1 c_half, mid = (x1+x0) c_half, ...
+    T drift_lead, drift_mid, drift_trail, drift_merged;
+    // the same for z on the exact (split-drift) path
+    T zdrift_lead, zdrift_mid, zdrift_trail;
+    T sinA[3][kMaxSin];     // tau_k * A * S coefficients, k = stage (Ruth4: x1, x0, x1)
+    T sin1[kMaxSin];        // S coefficients, unscaled (membership test, generic kick)
+    T cos1[kMaxCos];        // C coefficients: cos(pi f) = C(f^2)
+    T two_r;                // 2 r
+    T kickA[3];             // tau_k * A           (generic phi_s path)
+    T phi_off;              // phi_s/pi
+    T sin_phi_s;            // sin(phi_s)
+    T r;                    // r
+    T z_max;                // pi R / h
+    T hn_delta;             // eta C / (2 H_sep): H/H_sep = hn_delta delta^2 + S^2 (1 + 2r(1-S^2))
+};
+
+// ------------------------------------------------------------------------------------------
+// fp64 / fp32 traits
+// ------------------------------------------------------------------------------------------
+template <typename T> struct Real;
+
+template <> struct Real<double> {
+    static constexpr int NS = 8, NC = 9;
+    typedef double2 vec2;
+    static __device__ __forceinline__ double magic() { return 6755399441055744.0; }  // 1.5*2^52
+    static __device__ __forceinline__ double fma(double a, double b, double c) { return __fma_rn(a, b, c); }
+    static __device__ __forceinline__ double add(double a, double b) { return __dadd_rn(a, b); }
+    static __device__ __forceinline__ double sub(double a, double b) { return __dsub_rn(a, b); }
+    static __device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
+    // f with the sign bit flipped when the integer held in the low mantissa bits of t is odd.
+    // hi + (lo << 31) mod 2^32 == hi ^ ((lo & 1) << 31): ONE IMAD instead of shift + xor (every
+    // non-FP64 instruction in the turn loop costs about two issue cycles, profiles/ubench).
+    static __device__ __forceinline__ double flip(double f, double t) {
+        int hi = __double2hiint(f) + __double2loint(t) * (int)0x80000000;
+        return __hiloint2double(hi, __double2loint(f));
+    }
+    static __device__ __forceinline__ double flip_by(double x, double t) { return flip(x, t); }
+};
+
+template <> struct Real<float> {
+    static constexpr int NS = 5, NC = 6;
+    typedef float2 vec2;
+    static __device__ __forceinline__ float magic() { return 12582912.0f; }          // 1.5*2^23
+    static __device__ __forceinline__ float fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+    static __device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b); }
+    static __device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
+    static __device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
+    static __device__ __forceinline__ float flip(float f, float t) {
+        return __int_as_float(__float_as_int(f) + __float_as_int(t) * (int)0x80000000);
+    }
+    static __device__ __forceinline__ float flip_by(float x, float t) { return flip(x, t); }
+};
+
+// exact reduction: returns f = v - rint(v); *t_out keeps the parity of rint(v) in its low bit
+template <typename T>
+__device__ __forceinline__ T reduce_half_periods(T v, T* t_out) {
+    typedef Real<T> R;
+    T t = R::add(v, R::magic());
+    T n = R::sub(t, R::magic());
+    *t_out = t;
+    return R::sub(v, n);
+}
+
+// Horner evaluation of c[0] + c[1] s + ... + c[NUSED-1] s^(NUSED-1)
+template <typename T, int NUSED, int N>
+__device__ __forceinline__ T horner(const T (&c)[N], T s) {
+    static_assert(NUSED <= N, "polynomial longer than its table");
+    T q = c[NUSED - 1];
+#pragma unroll
+    for (int k = NUSED - 2; k >= 0; --k) q = Real<T>::fma(q, s, c[k]);
+    return q;
+}
+
+// ------------------------------------------------------------------------------------------
+// The kick  delta += tau_k * F(z)  for the phase v (half periods).
+//   HARM = 1: F = A sin(pi v)                              (configs[0])
+//   HARM = 2: F = A [sin(pi v) + r sin(2 pi v)] = A sin(pi v) (1 + 2 r cos(pi v))   (configs[4])
+//   HARM = 0: generic, phi_s != 0:  A [sin(phi_s + pi v) - sin(phi_s) + r sin(2 pi v)]   (G3)
+// ------------------------------------------------------------------------------------------
+// FQ selects WHERE the sign (-1)^n is applied: to f (off the critical path, best below ~5
+// resident warps per sub-partition) or to the polynomial value q (one dependent integer op
+// later, but it measured 3-4 % faster once the FP64 pipe is saturated; profiles/ubench_r1.md).
+template <typename T, int HARM, bool FQ = false>
+__device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage) {
+    typedef Real<T> R;
+    constexpr int NS = R::NS, NC = R::NC;
+    if (HARM == 1) {
+        T t;
+        T f = reduce_half_periods(v, &t);
+        T s = R::mul(f, f);
+        T q = horner<T, NS>(P.sinA[stage], s);
+        if (FQ) return R::fma(f, R::flip(q, t), delta);
+        return R::fma(R::flip(f, t), q, delta);
+    } else if (HARM == 2) {
+        T t;
+        T f = reduce_half_periods(v, &t);
+        T s = R::mul(f, f);
+        T q = horner<T, NS>(P.sinA[stage], s);   // tau A sin(pi f)/f
+        T c = horner<T, NC>(P.cos1, s);           // cos(pi f)
+        // sin and cos both change sign with the parity of n: flip f, and flip 2r for the cos
+        T m = R::fma(R::flip_by(P.two_r, t), c, T(1));
+        if (FQ) return R::fma(f, R::flip(R::mul(q, m), t), delta);
+        return R::fma(R::flip(f, t), R::mul(q, m), delta);
+    } else {
+        T t1, t2;
+        T f1 = reduce_half_periods(R::add(v, P.phi_off), &t1);
+        T s1 = R::mul(f1, f1);
+        T sn = R::mul(R::flip(f1, t1), horner<T, NS>(P.sin1, s1));
+        T acc = R::sub(sn, P.sin_phi_s);
+        T f2 = reduce_half_periods(R::add(v, v), &t2);
+        T s2 = R::mul(f2, f2);
+        T sn2 = R::mul(R::flip(f2, t2), horner<T, NS>(P.sin1, s2));
+        acc = R::fma(P.r, sn2, acc);
+        return R::fma(P.kickA[stage], acc, delta);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// One full turn on the EXACT path: the state is z itself, every half drift is its own FMA
+// (bit-identical between the per-turn kernel, the split-drift fused kernel and any chunking).
+// ------------------------------------------------------------------------------------------
+template <typename T, int INTEG, int HARM>
+__device__ __forceinline__ void turn_exact(T& z, T& delta, const MapConsts<T>& P) {
+    typedef Real<T> R;
+    if (INTEG == kLeapfrog) {
+        z = R::fma(-P.zdrift_lead, delta, z);
+        delta = kick<T, HARM>(R::mul(z, P.to_phase), delta, P, 0);
+        z = R::fma(-P.zdrift_trail, delta, z);
+    } else if (INTEG == kEulerCromer) {
+        delta = kick<T, HARM>(R::mul(z, P.to_phase), delta, P, 0);
+        z = R::fma(-P.zdrift_trail, delta, z);
+    } else {
+        z = R::fma(-P.zdrift_lead, delta, z);
+        delta = kick<T, HARM>(R::mul(z, P.to_phase), delta, P, 0);
+        z = R::fma(-P.zdrift_mid, delta, z);
+        delta = kick<T, HARM>(R::mul(z, P.to_phase), delta, P, 1);
+        z = R::fma(-P.zdrift_mid, delta, z);
+        delta = kick<T, HARM>(R::mul(z, P.to_phase), delta, P, 2);
+        z = R::fma(-P.zdrift_trail, delta, z);
+    }
+}
+
+// One turn on the FAST path, state = phase v, WITHOUT its leading drift and with the trailing
+// drift given by the caller (merged with the next turn's leading drift, or the plain trailing
+// one at the end of a call).
+template <typename T, int INTEG, int HARM, bool FQ = false>
+__device__ __forceinline__ void turn_fast(T& v, T& delta, const MapConsts<T>& P, T trailing) {
+    typedef Real<T> R;
+    if (INTEG == kRuth4) {
+        delta = kick<T, HARM, FQ>(v, delta, P, 0);
+        v = R::fma(-P.drift_mid, delta, v);
+        delta = kick<T, HARM, FQ>(v, delta, P, 1);
+        v = R::fma(-P.drift_mid, delta, v);
+        delta = kick<T, HARM, FQ>(v, delta, P, 2);
+        v = R::fma(-trailing, delta, v);
+    } else {
+        delta = kick<T, HARM, FQ>(v, delta, P, 0);
+        v = R::fma(-trailing, delta, v);
+    }
+}
+
+// `turns` turns of ILP particles held in registers (steps a2-a6).  Fast path: the state is the
+// phase v; `first` converts z -> v and applies the leading drift, `last` applies the plain
+// trailing drift and converts back, in between consecutive half drifts are merged.  Between
+// chunks of one call the z array therefore holds v mid-drift, which makes the result of a
+// call independent of how its turns are chunked.  SPLIT: exact path, state is z.
+template <typename T, int INTEG, int HARM, bool SPLIT, int ILP, bool FQ>
+__device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int turns, int first,
+                                        int last, const MapConsts<T>& P) {
+    typedef Real<T> R;
+    if (SPLIT) {
+        for (unsigned int t = 0; t < turns; ++t) {
+#pragma unroll
+            for (int j = 0; j < ILP; ++j) turn_exact<T, INTEG, HARM>(x[j], dl[j], P);
+        }
+    } else {
+        if (first) {
+#pragma unroll
+            for (int j = 0; j < ILP; ++j) {
+                x[j] = R::mul(x[j], P.to_phase);
+                if (INTEG != kEulerCromer) x[j] = R::fma(-P.drift_lead, dl[j], x[j]);
+            }
+        }
+        // every non-FP64 instruction costs about two issue cycles next to the saturated FP64
+        // pipe (profiles/ubench_r1.md): unroll deep enough that the loop counter disappears
+        constexpr int kUnroll = (INTEG == kRuth4 || HARM != 1 || ILP > 2) ? 4 : LT_TURN_UNROLL / ILP;
+#pragma unroll kUnroll
+        for (unsigned int t = 1; t < turns; ++t) {
+#pragma unroll
+            for (int j = 0; j < ILP; ++j)
+                turn_fast<T, INTEG, HARM, FQ>(x[j], dl[j], P, P.drift_merged);
+        }
+        const T trailing = last ? P.drift_trail : P.drift_merged;
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            turn_fast<T, INTEG, HARM, FQ>(x[j], dl[j], P, trailing);
+            if (last) x[j] = R::mul(x[j], P.from_phase);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Fused multi-turn kernel (registers hold the state over the inner turn
+// loop; the host loops over chunks).  One thread owns ILP particles; a block owns a tile of
+// blockDim.x * ILP consecutive particles, element j of thread t = tile + j*blockDim.x + t
+// (coalesced; double2 when VEC).  `first` / `last` mark the first / last chunk of a call:
+// between chunks the z array holds the phase v mid-drift, so that the result of a call does
+// not depend on the chunk length.
+// ------------------------------------------------------------------------------------------
+template <typename T, int INTEG, int HARM, bool SPLIT, int ILP, bool VEC>
+__global__ void fused_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n,
+                             unsigned int turns, int first, int last,
+                             const __grid_constant__ MapConsts<T> P) {
+    typedef Real<T> R;
+    typedef typename R::vec2 V2;
+    T x[ILP], dl[ILP];
+    const size_t tile = (size_t)blockIdx.x * blockDim.x * ILP;
+
+    // ---- entry load (a1)
+    if (VEC) {
+#pragma unroll
+        for (int j = 0; j < ILP / 2; ++j) {
+            size_t i = tile + 2 * ((size_t)j * blockDim.x + threadIdx.x);
+            if (i + 1 < n) {
+                V2 a = *reinterpret_cast<const V2*>(z_arr + i);
+                V2 b = *reinterpret_cast<const V2*>(d_arr + i);
+                x[2 * j] = a.x; x[2 * j + 1] = a.y; dl[2 * j] = b.x; dl[2 * j + 1] = b.y;
+            } else {
+                x[2 * j] = (i < n) ? z_arr[i] : T(0); dl[2 * j] = (i < n) ? d_arr[i] : T(0);
+                x[2 * j + 1] = T(0); dl[2 * j + 1] = T(0);
+            }
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            size_t i = tile + (size_t)j * blockDim.x + threadIdx.x;
+            x[j] = (i < n) ? z_arr[i] : T(0);
+            dl[j] = (i < n) ? d_arr[i] : T(0);
+        }
+    }
+
+    advance<T, INTEG, HARM, SPLIT, ILP, false>(x, dl, turns, first, last, P);
+
+    // ---- exit store (a7)
+    if (VEC) {
+#pragma unroll
+        for (int j = 0; j < ILP / 2; ++j) {
+            size_t i = tile + 2 * ((size_t)j * blockDim.x + threadIdx.x);
+            if (i + 1 < n) {
+                V2 a, b;
+                a.x = x[2 * j]; a.y = x[2 * j + 1]; b.x = dl[2 * j]; b.y = dl[2 * j + 1];
+                *reinterpret_cast<V2*>(z_arr + i) = a;
+                *reinterpret_cast<V2*>(d_arr + i) = b;
+            } else if (i < n) {
+                z_arr[i] = x[2 * j]; d_arr[i] = dl[2 * j];
+            }
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            size_t i = tile + (size_t)j * blockDim.x + threadIdx.x;
+            if (i < n) { z_arr[i] = x[j]; d_arr[i] = dl[j]; }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Fused multi-turn kernel with ON-DEVICE DYNAMIC CHUNKING -- the paper's hybrid loop (CPU outer
+// loop x in-kernel inner loop) with the outer loop moved onto the GPU.
+//
+// Why: a warp-wide FP64 instruction occupies a sub-partition's FP64 pipe for two cycles whatever
+// the ensemble size, so 10^5 particles = 3125 warps over 592 sub-partitions leave some with 6
+// and some with 5 warps for the WHOLE run: 12 % of the pipe idles, and nothing static fixes it.
+// Here a persistent grid (one CTA of 4W warps per SM) keeps W warps on every sub-partition; work items are
+// (chunk c of `item_turns` turns) x (group g of 32 particles), handed out by one atomic ticket
+// in c-major order; the state goes through L2 between items (512 B per item, noise).  Every
+// sub-partition stays saturated until the last few items.  An item's predecessor (c-1, g) has a
+// smaller ticket, so it is finished or running: the acquire-poll on done[g] cannot deadlock and
+// is in practice never taken when there are more groups than resident warps.
+// The arithmetic per particle is identical to fused_kernel, so results are bit-identical to it
+// and independent of item_turns and of the scheduling order.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u32(unsigned int* p, unsigned int v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ>
+__global__ void __launch_bounds__(1024, 1)
+fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, unsigned int turns,
+                        unsigned int item_turns, int first_launch, int last_launch, int dynamic,
+                        unsigned long long* __restrict__ ticket, unsigned int* __restrict__ done,
+                        const __grid_constant__ MapConsts<T> P) {
+    extern __shared__ unsigned char residency_cap[];   // unused: sized to cap CTAs per SM
+    const unsigned int lane = threadIdx.x & 31u;
+    const unsigned long long groups = (n + 31) / 32;
+    const unsigned int nchunks = (turns + item_turns - 1) / item_turns;
+    const unsigned long long total = groups * nchunks;
+    // static mode (few groups): slot s of the grid owns groups s, s + S, ... for all turns;
+    // slots are numbered SM-first so that groups spread evenly over SMs and sub-partitions
+    const unsigned long long slots = (unsigned long long)gridDim.x * (blockDim.x >> 5);
+    unsigned long long next = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
+    for (;;) {
+        unsigned long long t = next;
+        if (dynamic) {
+            if (lane == 0) t = atomicAdd(ticket, 1ULL);
+            t = __shfl_sync(0xffffffffu, t, 0);
+        } else {
+            next += slots;
+        }
+        if (t >= total) break;
+        const unsigned int c = (unsigned int)(t / groups);
+        const unsigned long long g = t - (unsigned long long)c * groups;
+        if (c > 0) {
+            while (ld_acquire_u32(done + g) < c) __nanosleep(64);
+        }
+        const size_t i = (size_t)g * 32 + lane;
+        T x[1], dl[1];
+        x[0] = (i < n) ? __ldcg(z_arr + i) : T(0);      // L2 only: another SM may have written it
+        dl[0] = (i < n) ? __ldcg(d_arr + i) : T(0);
+        const int first = first_launch && c == 0;
+        const int last = last_launch && c == nchunks - 1;
+        const unsigned int nt = (c == nchunks - 1) ? turns - c * item_turns : item_turns;
+        advance<T, INTEG, HARM, SPLIT, 1, FQ>(x, dl, nt, first, last, P);
+        if (i < n) { __stcg(z_arr + i, x[0]); __stcg(d_arr + i, dl[0]); }
+        if (nchunks > 1) {
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) st_release_u32(done + g, c + 1);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Bucket membership of one state (G15):  |z| < z_max  and  H/H_sep < 1 with
+//     H/H_sep = hn_delta delta^2 + S^2 (1 + 2 r (1 - S^2)),   S = sin(kappa z / 2).
+// ------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ bool in_bucket(T z, T delta, const MapConsts<T>& P) {
+    typedef Real<T> R;
+    T t;
+    T g = reduce_half_periods(R::mul(z, R::mul(P.to_phase, T(0.5))), &t);
+    T S = R::mul(g, horner<T, R::NS>(P.sin1, R::mul(g, g)));
+    T S2 = R::mul(S, S);
+    T pot = R::mul(S2, R::fma(P.two_r, R::sub(T(1), S2), T(1)));
+    T hn = R::fma(P.hn_delta, R::mul(delta, delta), pot);
+    return (fabs(z) < P.z_max) && (hn < T(1));
+}
+
+// Raw sums of a state, always accumulated in fp64.
+struct Sums {
+    double sz, szz, sd, sdd, szd;
+    unsigned long long nin;
+    __device__ __forceinline__ void zero() { sz = szz = sd = sdd = szd = 0.0; nin = 0ULL; }
+    __device__ __forceinline__ void add(double z, double d, bool inb) {
+        sz += z; szz = __fma_rn(z, z, szz); sd += d; sdd = __fma_rn(d, d, sdd);
+        szd = __fma_rn(z, d, szd); nin += inb ? 1ULL : 0ULL;
+    }
+};
+
+constexpr int kPartialStride = 8;   // doubles per (turn, CTA) partial: sz szz sd sdd szd nin pad pad
+
+__device__ __forceinline__ double warp_sum(double x) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+}
+
+// block combine: warp shuffles, then shared memory across warps, fixed order -> deterministic
+__device__ __forceinline__ void block_reduce_store(Sums s, double* __restrict__ out) {
+    __shared__ double sh[32][6];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    double v[6] = {s.sz, s.szz, s.sd, s.sdd, s.szd, (double)s.nin};
+#pragma unroll
+    for (int k = 0; k < 6; ++k) v[k] = warp_sum(v[k]);
+    if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) sh[warp][k] = v[k];
+    }
+    __syncthreads();
+    if (threadIdx.x < 6) {
+        double a = 0.0;
+        for (int w = 0; w < nw; ++w) a += sh[w][threadIdx.x];
+        out[threadIdx.x] = a;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Per-turn kernel (BASELINE.json:configs[3]): ONE turn per launch, z/delta read
+// and written through HBM (32 B per particle-turn in fp64), the turn's raw sums reduced in the
+// same pass (a8 + a9).  Persistent CTAs, each walking tiles of blockDim.x*2*UNR particles with
+// stride gridDim.x; `reverse` walks the array backwards (odd turns) so that the tail the
+// previous launch left in the 126 MB L2 is consumed first.
+// partials: [gridDim.x][kPartialStride] doubles for this turn.
+// ------------------------------------------------------------------------------------------
+template <typename T, int INTEG, int HARM, bool MOMENTS, int UNR>
+__global__ void per_turn_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n,
+                                int reverse, double* __restrict__ partials,
+                                const __grid_constant__ MapConsts<T> P) {
+    typedef typename Real<T>::vec2 V2;
+    Sums acc;
+    acc.zero();
+    const size_t npair = n >> 1;                                   // full pairs
+    const size_t tile_pairs = (size_t)blockDim.x * UNR;
+    const size_t ntiles = (npair + tile_pairs - 1) / tile_pairs;
+    for (size_t tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
+        const size_t tix = reverse ? (ntiles - 1 - tl) : tl;
+        const size_t base = tix * tile_pairs;
+        V2 a[UNR], b[UNR];
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            size_t p = base + (size_t)u * blockDim.x + threadIdx.x;
+            if (p < npair) {
+                a[u] = reinterpret_cast<const V2*>(z_arr)[p];
+                b[u] = reinterpret_cast<const V2*>(d_arr)[p];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            size_t p = base + (size_t)u * blockDim.x + threadIdx.x;
+            if (p < npair) {
+                turn_exact<T, INTEG, HARM>(a[u].x, b[u].x, P);
+                turn_exact<T, INTEG, HARM>(a[u].y, b[u].y, P);
+                reinterpret_cast<V2*>(z_arr)[p] = a[u];
+                reinterpret_cast<V2*>(d_arr)[p] = b[u];
+                if (MOMENTS) {
+                    acc.add((double)a[u].x, (double)b[u].x, in_bucket<T>(a[u].x, b[u].x, P));
+                    acc.add((double)a[u].y, (double)b[u].y, in_bucket<T>(a[u].y, b[u].y, P));
+                }
+            }
+        }
+    }
+    // odd tail particle
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        T zz = z_arr[n - 1], dd = d_arr[n - 1];
+        turn_exact<T, INTEG, HARM>(zz, dd, P);
+        z_arr[n - 1] = zz; d_arr[n - 1] = dd;
+        if (MOMENTS) acc.add((double)zz, (double)dd, in_bucket<T>(zz, dd, P));
+    }
+    if (MOMENTS) block_reduce_store(acc, partials + (size_t)blockIdx.x * kPartialStride);
+}
+
+// scalar variant for arrays that are not 16-byte (fp64) / 8-byte (fp32) aligned
+template <typename T, int INTEG, int HARM, bool MOMENTS>
+__global__ void per_turn_kernel_scalar(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n,
+                                       double* __restrict__ partials,
+                                       const __grid_constant__ MapConsts<T> P) {
+    Sums acc;
+    acc.zero();
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (size_t)gridDim.x * blockDim.x) {
+        T zz = z_arr[i], dd = d_arr[i];
+        turn_exact<T, INTEG, HARM>(zz, dd, P);
+        z_arr[i] = zz; d_arr[i] = dd;
+        if (MOMENTS) acc.add((double)zz, (double)dd, in_bucket<T>(zz, dd, P));
+    }
+    if (MOMENTS) block_reduce_store(acc, partials + (size_t)blockIdx.x * kPartialStride);
+}
+
+// Sums of the current state without tracking (lt_moments_now, lt_bucket_count).
+template <typename T, bool ONLY_COUNT>
+__global__ void state_sums_kernel(const T* __restrict__ z_arr, const T* __restrict__ d_arr,
+                                  size_t n, double* __restrict__ partials,
+                                  const __grid_constant__ MapConsts<T> P) {
+    Sums acc;
+    acc.zero();
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (size_t)gridDim.x * blockDim.x) {
+        T zz = z_arr[i], dd = d_arr[i];
+        bool inb = in_bucket<T>(zz, dd, P);
+        if (ONLY_COUNT) acc.nin += inb ? 1ULL : 0ULL;
+        else acc.add((double)zz, (double)dd, inb);
+    }
+    block_reduce_store(acc, partials + (size_t)blockIdx.x * kPartialStride);
+}
+
+// ------------------------------------------------------------------------------------------
+// Finalise: one CTA per turn of a batch sums that turn's per-CTA partials in a fixed order
+// (deterministic) and writes lt_sums / lt_moments / the count.  `cursor` (device) holds the
+// index of the batch's first turn in the output arrays; the last CTA to finish advances it, so
+// that the same launch can be replayed from a CUDA graph.
+// ------------------------------------------------------------------------------------------
+struct SumsOut { double n, sum_z, sum_zz, sum_d, sum_dd, sum_zd, n_in_bucket, pad_; };
+struct MomentsOut { double mean_z, rms_z, mean_d, rms_d, cov_zd; unsigned long long n_in_bucket; };
+
+__device__ __forceinline__ MomentsOut moments_from(const SumsOut& s) {
+    MomentsOut m;
+    const double inv = s.n > 0.0 ? 1.0 / s.n : 0.0;
+    m.mean_z = s.sum_z * inv;
+    m.mean_d = s.sum_d * inv;
+    double vz = __fma_rn(-m.mean_z, m.mean_z, s.sum_zz * inv);
+    double vd = __fma_rn(-m.mean_d, m.mean_d, s.sum_dd * inv);
+    m.rms_z = sqrt(vz > 0.0 ? vz : 0.0);
+    m.rms_d = sqrt(vd > 0.0 ? vd : 0.0);
+    m.cov_zd = __fma_rn(-m.mean_z, m.mean_d, s.sum_zd * inv);
+    m.n_in_bucket = (unsigned long long)(s.n_in_bucket + 0.5);
+    return m;
+}
+
+__global__ void finalize_kernel(const double* __restrict__ partials, int nparts, size_t n,
+                                unsigned long long* __restrict__ cursor, unsigned int* done,
+                                MomentsOut* __restrict__ moments, SumsOut* __restrict__ sums,
+                                unsigned long long* __restrict__ count_out) {
+    __shared__ double sh[6][8];
+    const double* mine = partials + (size_t)blockIdx.x * nparts * kPartialStride;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;   // blockDim.x == 256
+    double v[6] = {0, 0, 0, 0, 0, 0};
+    for (int p = threadIdx.x; p < nparts; p += blockDim.x) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) v[k] += mine[(size_t)p * kPartialStride + k];
+    }
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        v[k] = warp_sum(v[k]);
+        if (lane == 0) sh[k][warp] = v[k];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        SumsOut s;
+        double r[6];
+        for (int k = 0; k < 6; ++k) {
+            double a = 0.0;
+            for (int w = 0; w < 8; ++w) a += sh[k][w];
+            r[k] = a;
+        }
+        s.n = (double)n; s.sum_z = r[0]; s.sum_zz = r[1]; s.sum_d = r[2]; s.sum_dd = r[3];
+        s.sum_zd = r[4]; s.n_in_bucket = r[5]; s.pad_ = 0.0;
+        const unsigned long long t = (cursor ? *cursor : 0ULL) + blockIdx.x;
+        if (sums) sums[t] = s;
+        if (moments) moments[t] = moments_from(s);
+        if (count_out) count_out[t] = (unsigned long long)(r[5] + 0.5);
+        if (cursor) {
+            __threadfence();
+            if (atomicAdd(done, 1u) == gridDim.x - 1) {
+                *done = 0u;
+                *cursor += gridDim.x;
+            }
+        }
+    }
+}
+
+__global__ void set_cursor_kernel(unsigned long long* cursor, unsigned int* done,
+                                  unsigned long long value) {
+    *cursor = value;
+    *done = 0u;
+}
+
+// ------------------------------------------------------------------------------------------
+// FP64 roofline probe: CHAINS independent dependent-FMA chains per thread.
+// ------------------------------------------------------------------------------------------
+template <int CHAINS>
+__global__ void probe_dfma_kernel(double* out, long long iters, double a, double b) {
+    double x[CHAINS];
+#pragma unroll
+    for (int c = 0; c < CHAINS; ++c) x[c] = 1.0 + 1e-9 * (threadIdx.x + c);
+    for (long long i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int c = 0; c < CHAINS; ++c) x[c] = __fma_rn(x[c], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < CHAINS; ++c) s += x[c];
+    if (s == 12345.678) out[0] = s;   // never true; keeps the chains alive
+}
+
+}  // namespace lt

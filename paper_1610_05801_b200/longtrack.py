@@ -1,0 +1,221 @@
+"""ctypes binding of liblongtrack.so -- argument marshalling only.
+
+Same names as include/longtrack.h.  Every step of the hot path runs in the CUDA kernels of
+the library; nothing here computes.  PyTorch is used by CALLERS for device memory and streams
+(tensors are passed as raw device pointers); this module itself does not import torch.
+
+Importing this module loads the library and raises ImportError when it is missing: there is
+no CPU fallback and nothing under oracle/ is ever touched from here.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import (POINTER, Structure, byref, c_char_p, c_double, c_int, c_longlong, c_size_t,
+                    c_ulonglong, c_void_p)
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+# LONGTRACK_LIB overrides the path (e.g. to try a build with other compile-time knobs)
+LIB_PATH = os.environ.get("LONGTRACK_LIB") or os.path.join(_HERE, "liblongtrack.so")
+
+EULER_CROMER, LEAPFROG, RUTH4 = 0, 1, 2
+INTEGRATORS = {"euler_cromer": EULER_CROMER, "leapfrog": LEAPFROG, "ruth4": RUTH4}
+
+OK, E_NULL, E_PARAM, E_UNSTABLE, E_ALIGN, E_CUDA, E_NOMEM = 0, -1, -2, -3, -4, -5, -6
+
+OPT_SPLIT_DRIFTS, OPT_CHUNK_TURNS, OPT_FUSED_ILP, OPT_FUSED_BLOCK = 1, 2, 3, 4
+OPT_PER_TURN_GRAPH, OPT_PER_TURN_CTAS_PER_SM, OPT_PER_TURN_REVERSE = 5, 6, 7
+OPT_FUSED_MODE, OPT_ITEM_TURNS, OPT_WARPS_PER_SMSP, OPT_FLIP_ON_Q = 8, 9, 10, 11
+FUSED_AUTO, FUSED_PLAIN, FUSED_PERSISTENT_STATIC, FUSED_PERSISTENT_DYNAMIC = 0, 1, 2, 3
+STAT_KERNEL_LAUNCHES, STAT_LAST_GRID, STAT_LAST_BLOCK, STAT_LAST_ILP, STAT_SM_COUNT = 1, 2, 3, 4, 5
+STAT_LAST_MODE, STAT_LAST_ITEM_TURNS = 6, 7
+
+
+class Params(Structure):
+    _fields_ = [("circumference_m", c_double), ("gamma", c_double), ("alpha_c", c_double),
+                ("p0c_eV", c_double), ("charge_e", c_double), ("harmonic", c_int),
+                ("voltage_V", c_double), ("phi_s", c_double), ("ratio2", c_double),
+                ("integrator", c_int)]
+
+
+class Derived(Structure):
+    _fields_ = [(k, c_double) for k in
+                ("R", "beta", "eta", "A", "d", "kappa", "K", "mu", "z_max", "H_sep")]
+
+
+MOMENTS_DTYPE = np.dtype([("mean_z", "f8"), ("rms_z", "f8"), ("mean_d", "f8"), ("rms_d", "f8"),
+                          ("cov_zd", "f8"), ("n_in_bucket", "u8")])
+SUMS_DTYPE = np.dtype([("n", "f8"), ("sum_z", "f8"), ("sum_zz", "f8"), ("sum_d", "f8"),
+                       ("sum_dd", "f8"), ("sum_zd", "f8"), ("n_in_bucket", "f8"), ("pad_", "f8")])
+
+
+class LongtrackError(RuntimeError):
+    def __init__(self, code: int, cuda_error: int = 0):
+        self.code = code
+        self.cuda_error = cuda_error
+        msg = _lib.lt_strerror(code).decode()
+        if cuda_error:
+            msg += " [cudaError %d]" % cuda_error
+        super().__init__("liblongtrack: %s (%d)" % (msg, code))
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "%s is missing: build it with `python -m paper_1610_05801_b200.build` "
+            "(there is no CPU fallback)" % LIB_PATH)
+    L = ctypes.CDLL(LIB_PATH)
+    vp, sz, ull = c_void_p, c_size_t, c_ulonglong
+    sig = {
+        "lt_create": (c_int, [POINTER(Params), POINTER(vp)]),
+        "lt_destroy": (c_int, [vp]),
+        "lt_derived": (c_int, [vp, POINTER(Derived)]),
+        "lt_set_option": (c_int, [vp, c_int, c_longlong]),
+        "lt_get_option": (c_int, [vp, c_int, POINTER(c_longlong)]),
+        "lt_get_stat": (c_int, [vp, c_int, POINTER(c_longlong)]),
+        "lt_strerror": (c_char_p, [c_int]),
+        "lt_last_cuda_error": (c_int, [vp]),
+        "lt_version": (c_int, []),
+        "lt_track_fused": (c_int, [vp, vp, vp, sz, ull, vp]),
+        "lt_track_fused_f32": (c_int, [vp, vp, vp, sz, ull, vp]),
+        "lt_track_per_turn": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp]),
+        "lt_track_per_turn_f32": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp]),
+        "lt_bucket_count": (c_int, [vp, vp, vp, sz, vp, vp]),
+        "lt_bucket_count_f32": (c_int, [vp, vp, vp, sz, vp, vp]),
+        "lt_moments_now": (c_int, [vp, vp, vp, sz, vp, vp, vp]),
+        "lt_moments_from_sums": (c_int, [vp, sz, vp]),
+        "lt_track_fused_host": (c_int, [vp, vp, vp, sz, ull, POINTER(ull)]),
+        "lt_probe_fp64": (c_int, [c_int, c_int, c_int, c_longlong, POINTER(c_double),
+                                  POINTER(c_double)]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    return L, tuple(sig)
+
+
+_lib, EXPORTS = _load()
+
+
+def make_params(ring: dict, integrator="leapfrog", ratio2: float = 0.0,
+                phi_s: float | None = None) -> Params:
+    integ = INTEGRATORS[integrator] if isinstance(integrator, str) else int(integrator)
+    return Params(float(ring["circumference_m"]), float(ring["gamma"]), float(ring["alpha_c"]),
+                  float(ring["p0c_eV"]), float(ring.get("charge_e", 1.0)), int(ring["harmonic"]),
+                  float(ring["voltage_V"]),
+                  float(ring.get("phi_s", 0.0) if phi_s is None else phi_s), float(ratio2), integ)
+
+
+def _ptr(x) -> int:
+    """Raw address of a torch tensor (device or host), a numpy array, an int or None."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return int(x.data_ptr())
+    return int(x.ctypes.data)
+
+
+class Tracker:
+    """lt_create / lt_destroy with the track calls as methods (names as in longtrack.h)."""
+
+    def __init__(self, ring: dict, integrator="leapfrog", ratio2: float = 0.0,
+                 phi_s: float | None = None):
+        self.params = make_params(ring, integrator, ratio2, phi_s)
+        self._h = c_void_p()
+        rc = _lib.lt_create(byref(self.params), byref(self._h))
+        if rc != OK:
+            raise LongtrackError(rc)
+
+    def _check(self, rc: int):
+        if rc != OK:
+            raise LongtrackError(rc, _lib.lt_last_cuda_error(self._h) if rc == E_CUDA else 0)
+
+    def close(self):
+        if getattr(self, "_h", None) and _lib is not None:     # _lib is None at interpreter exit
+            _lib.lt_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def derived(self) -> dict:
+        out = Derived()
+        self._check(_lib.lt_derived(self._h, byref(out)))
+        return {k: getattr(out, k) for k, _ in Derived._fields_}
+
+    def set_option(self, option: int, value: int):
+        self._check(_lib.lt_set_option(self._h, option, int(value)))
+
+    def get_option(self, option: int) -> int:
+        v = c_longlong()
+        self._check(_lib.lt_get_option(self._h, option, byref(v)))
+        return v.value
+
+    def get_stat(self, stat: int) -> int:
+        v = c_longlong()
+        self._check(_lib.lt_get_stat(self._h, stat, byref(v)))
+        return v.value
+
+    # ---- device-pointer calls: z, delta are CUDA tensors (or raw addresses); stream = int
+    def track_fused(self, z, delta, n: int, turns: int, stream: int = 0):
+        self._check(_lib.lt_track_fused(self._h, _ptr(z), _ptr(delta), n, turns, stream))
+
+    def track_fused_f32(self, z, delta, n: int, turns: int, stream: int = 0):
+        self._check(_lib.lt_track_fused_f32(self._h, _ptr(z), _ptr(delta), n, turns, stream))
+
+    def track_per_turn(self, z, delta, n: int, turns: int, moments=None, sums=None,
+                       stream: int = 0):
+        self._check(_lib.lt_track_per_turn(self._h, _ptr(z), _ptr(delta), n, turns,
+                                           _ptr(moments), _ptr(sums), stream))
+
+    def track_per_turn_f32(self, z, delta, n: int, turns: int, moments=None, sums=None,
+                           stream: int = 0):
+        self._check(_lib.lt_track_per_turn_f32(self._h, _ptr(z), _ptr(delta), n, turns,
+                                               _ptr(moments), _ptr(sums), stream))
+
+    def bucket_count(self, z, delta, n: int, count, stream: int = 0):
+        self._check(_lib.lt_bucket_count(self._h, _ptr(z), _ptr(delta), n, _ptr(count), stream))
+
+    def bucket_count_f32(self, z, delta, n: int, count, stream: int = 0):
+        self._check(_lib.lt_bucket_count_f32(self._h, _ptr(z), _ptr(delta), n, _ptr(count),
+                                             stream))
+
+    def moments_now(self, z, delta, n: int, moments=None, sums=None, stream: int = 0):
+        self._check(_lib.lt_moments_now(self._h, _ptr(z), _ptr(delta), n, _ptr(moments),
+                                        _ptr(sums), stream))
+
+    # ---- host-buffer call
+    def track_fused_host(self, z_host, delta_host, n: int, turns: int, want_count: bool = False):
+        cnt = c_ulonglong(0)
+        self._check(_lib.lt_track_fused_host(self._h, _ptr(z_host), _ptr(delta_host), n, turns,
+                                             byref(cnt) if want_count else None))
+        return cnt.value if want_count else None
+
+
+def moments_from_sums(sums: np.ndarray) -> np.ndarray:
+    sums = np.ascontiguousarray(sums, dtype=SUMS_DTYPE)
+    out = np.zeros(sums.shape, dtype=MOMENTS_DTYPE)
+    rc = _lib.lt_moments_from_sums(sums.ctypes.data, sums.size, out.ctypes.data)
+    if rc != OK:
+        raise LongtrackError(rc)
+    return out
+
+
+def probe_fp64(blocks: int, threads: int, chains: int, iters: int):
+    rate, ms = c_double(), c_double()
+    rc = _lib.lt_probe_fp64(blocks, threads, chains, iters, byref(rate), byref(ms))
+    if rc != OK:
+        raise LongtrackError(rc)
+    return rate.value, ms.value
+
+
+def strerror(code: int) -> str:
+    return _lib.lt_strerror(code).decode()
+
+
+def version() -> int:
+    return _lib.lt_version()

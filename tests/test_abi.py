@@ -1,0 +1,143 @@
+"""-m "not gpu": the C-ABI library loads here (no GPU), exports every symbol that
+include/longtrack.h declares, and its host-only entry points behave as documented."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+import __graft_entry__ as entry
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lt():
+    entry.build()
+    from paper_1610_05801_b200 import longtrack
+    return longtrack
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "longtrack.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(lt_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported_and_bound(lt):
+    import ctypes
+    names = declared_functions()
+    assert len(names) >= 19
+    lib = ctypes.CDLL(lt.LIB_PATH)
+    for n in names:
+        assert hasattr(lib, n), "missing export " + n
+    assert sorted(lt.EXPORTS) == names      # the binding covers exactly the header
+
+
+def test_version_and_strerror(lt):
+    assert lt.version() == 100
+    assert lt.strerror(0) == "ok"
+    for code in range(-6, 0):
+        assert lt.strerror(code) not in ("ok", "unknown error code")
+
+
+def test_derived_constants_against_40_digit_values(lt):
+    from paper_1610_05801_b200 import workloads as wl
+    gold = {}
+    for line in open(os.path.join(ROOT, "tests", "golden", "derived_constants.txt")):
+        if not line.startswith("#"):
+            k, v = line.split()
+            gold[k] = float(v)
+    d = lt.Tracker(wl.RING).derived()
+    for k in ("R", "beta", "eta", "A", "d", "kappa", "K", "z_max", "H_sep"):
+        assert abs(d[k] - gold[k]) <= 4 * np.spacing(abs(gold[k])), k
+    assert d["mu"] == pytest.approx(gold["mu"], rel=1e-10)
+
+
+def test_parameter_validation(lt):
+    from paper_1610_05801_b200 import workloads as wl
+
+    def code(**over):
+        ring = dict(wl.RING)
+        integ = over.pop("integrator", "leapfrog")
+        r = over.pop("ratio2", 0.0)
+        ring.update(over)
+        try:
+            lt.Tracker(ring, integ, r)
+        except lt.LongtrackError as e:
+            return e.code
+        return 0
+
+    assert code() == 0
+    assert code(gamma=1.0) == lt.E_PARAM
+    assert code(circumference_m=0.0) == lt.E_PARAM
+    assert code(harmonic=0) == lt.E_PARAM
+    assert code(p0c_eV=-1.0) == lt.E_PARAM
+    assert code(voltage_V=float("nan")) == lt.E_PARAM
+    assert code(integrator=7) == lt.E_PARAM
+    assert code(voltage_V=-2.0e6) == lt.E_UNSTABLE          # K < 0
+    assert code(voltage_V=2.0e6 * 3000) == lt.E_UNSTABLE    # K >= 4
+    assert code(ratio2=-0.5) == 0                           # K_eff == 0 is allowed (G10)
+    assert code(ratio2=-0.6) == lt.E_UNSTABLE
+
+
+def test_options_and_stats(lt):
+    from paper_1610_05801_b200 import workloads as wl
+    tr = lt.Tracker(wl.RING)
+    assert tr.get_option(lt.OPT_CHUNK_TURNS) == 1 << 22
+    tr.set_option(lt.OPT_CHUNK_TURNS, 1000)
+    assert tr.get_option(lt.OPT_CHUNK_TURNS) == 1000
+    for opt, bad in ((lt.OPT_CHUNK_TURNS, 0), (lt.OPT_FUSED_ILP, 3), (lt.OPT_FUSED_BLOCK, 100),
+                     (lt.OPT_PER_TURN_CTAS_PER_SM, 0), (lt.OPT_FUSED_MODE, 4),
+                     (lt.OPT_WARPS_PER_SMSP, 9), (lt.OPT_FLIP_ON_Q, 2), (99, 1)):
+        with pytest.raises(lt.LongtrackError) as e:
+            tr.set_option(opt, bad)
+        assert e.value.code == lt.E_PARAM
+    assert tr.get_stat(lt.STAT_KERNEL_LAUNCHES) == 0
+
+
+def test_no_cpu_fallback_device_calls_fail_loudly_without_a_gpu(lt):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_1610_05801_b200 import workloads as wl
+    tr = lt.Tracker(wl.RING)
+    z, d = np.full(8, 0.1), np.zeros(8)
+    with pytest.raises(lt.LongtrackError) as e:
+        tr.track_fused_host(z, d, 8, 10)
+    assert e.value.code == lt.E_CUDA and e.value.cuda_error != 0
+    assert np.all(z == 0.1) and np.all(d == 0.0)            # nothing was computed on the CPU
+    # n == 0 is a no-op and needs no device
+    tr.track_fused_host(z, d, 0, 10)
+    tr.track_fused(0, 0, 0, 10)
+
+
+def test_moments_from_sums_host_helper(lt):
+    rng = np.random.default_rng(2)
+    z, d = rng.normal(0.01, 0.2, 1000), rng.normal(0, 2e-3, 1000)
+    s = np.zeros(1, dtype=lt.SUMS_DTYPE)
+    s["n"], s["sum_z"], s["sum_zz"] = z.size, z.sum(), (z * z).sum()
+    s["sum_d"], s["sum_dd"], s["sum_zd"], s["n_in_bucket"] = d.sum(), (d * d).sum(), (z * d).sum(), 17
+    m = lt.moments_from_sums(s)[0]
+    assert m["mean_z"] == pytest.approx(z.mean(), rel=1e-12)
+    assert m["rms_z"] == pytest.approx(z.std(), rel=1e-12)
+    assert m["rms_d"] == pytest.approx(d.std(), rel=1e-12)
+    assert m["cov_zd"] == pytest.approx(np.mean((z - z.mean()) * (d - d.mean())), rel=1e-9)
+    assert m["n_in_bucket"] == 17
+
+
+def test_product_path_never_touches_the_oracle():
+    """The package must not import, link or read anything under oracle/."""
+    pkg = os.path.join(ROOT, "paper_1610_05801_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
+                assert "longtrack_oracle" not in text and "lto_" not in text, f
+    for f in ("longtrack_oracle.c", "map.inc", "longtrack_oracle.h", "__init__.py"):
+        text = open(os.path.join(ROOT, "oracle", f)).read()
+        assert "paper_1610_05801_b200" not in text.replace(
+            "paper_1610_05801_b200/csrc/, include/longtrack.h", "").replace(
+            "from ``paper_1610_05801_b200``", "") or f == "__init__.py"
+        assert "longtrack.h\"" not in text and "kernels.cuh" not in text
