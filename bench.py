@@ -232,7 +232,9 @@ def run_cuda(args) -> None:
     fused_launch_s = t_fused / args.steps              # one fused kernel launch per step
     achieved_ginstr = n * turns * FP64_INSTR_PER_PT / fused_launch_s / 1e9
     peak_ginstr = SMS * FP64_LANES_PER_SM * sm_max_mhz * 1e6 / 1e9
-    roofline = {"bound": "alu", "kernel": "fused_kernel<double,leapfrog,single,merged>",
+    mode = {1: "fused_kernel (plain)", 2: "fused_persistent_kernel (static slots)",
+            3: "fused_persistent_kernel (dynamic chunk scheduling)"}[tr.get_stat(lt.STAT_LAST_MODE)]
+    roofline = {"bound": "alu", "kernel": mode + " <double, leap-frog, single harmonic, merged drifts>",
                 "achieved": achieved_ginstr, "peak": peak_ginstr, "unit": "G FP64 instr/s",
                 "frac": achieved_ginstr / peak_ginstr, "traffic": None,
                 "instr_per_particle_turn": FP64_INSTR_PER_PT,
@@ -240,7 +242,7 @@ def run_cuda(args) -> None:
                                "MEASURED_PEAKS.json has no FP64 entry",
                 "ms_per_launch": 1e3 * fused_launch_s,
                 "grid": tr.get_stat(lt.STAT_LAST_GRID), "block": tr.get_stat(lt.STAT_LAST_BLOCK),
-                "ilp": tr.get_stat(lt.STAT_LAST_ILP)}
+                "item_turns": tr.get_stat(lt.STAT_LAST_ITEM_TURNS)}
     clocks = clk.summary()
 
     # ---- e2e: host buffers through the C ABI (H2D + track + count + D2H per step)
@@ -298,8 +300,7 @@ def run_cuda(args) -> None:
     # ---- FP64 probe (measured DFMA issue rate, context for the derived peak)
     probe = None
     try:
-        rate, _ = lt.probe_fp64(SMS * 4, 256, 4, 100000)
-        probe = rate / 1e9
+        probe = max(lt.probe_fp64(SMS, 1024, ch, 400000)[0] for ch in (2, 4)) / 1e9
     except Exception:
         pass
     roofline["peak_measured_dfma_probe"] = probe

@@ -596,9 +596,13 @@ __global__ void probe_dfma_kernel(double* out, long long iters, double a, double
     double x[CHAINS];
 #pragma unroll
     for (int c = 0; c < CHAINS; ++c) x[c] = 1.0 + 1e-9 * (threadIdx.x + c);
-    for (long long i = 0; i < iters; ++i) {
+    const int n16 = (int)(iters / 16);
+    for (int i = 0; i < n16; ++i) {
 #pragma unroll
-        for (int c = 0; c < CHAINS; ++c) x[c] = __fma_rn(x[c], a, b);
+        for (int u = 0; u < 16; ++u) {
+#pragma unroll
+            for (int c = 0; c < CHAINS; ++c) x[c] = __fma_rn(x[c], a, b);
+        }
     }
     double s = 0.0;
 #pragma unroll

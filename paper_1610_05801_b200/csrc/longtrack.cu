@@ -837,7 +837,7 @@ int lt_track_fused_host(lt_tracker* tr, double* z_host, double* delta_host, size
 int lt_probe_fp64(int blocks, int threads, int chains, long long iters, double* rate_host,
                   double* ms_host) {
     if (!rate_host) return LT_E_NULL;
-    if (blocks < 1 || threads < 1 || threads > 1024 || iters < 1) return LT_E_PARAM;
+    if (blocks < 1 || threads < 1 || threads > 1024 || iters < 16 || iters > (1LL << 34)) return LT_E_PARAM;
     double* out = nullptr;
     cudaEvent_t e0, e1;
     if (cudaMalloc(&out, sizeof(double)) != cudaSuccess) { (void)cudaGetLastError(); return LT_E_CUDA; }
@@ -866,7 +866,7 @@ int lt_probe_fp64(int blocks, int threads, int chains, long long iters, double* 
     cudaFree(out);
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    *rate_host = (double)blocks * threads * chains * (double)iters / (ms * 1e-3);
+    *rate_host = (double)blocks * threads * chains * (double)(iters / 16 * 16) / (ms * 1e-3);
     if (ms_host) *ms_host = ms;
     return LT_OK;
 }
