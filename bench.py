@@ -39,6 +39,10 @@ UNIT = "particle-turns/s"
 FP64_INSTR_PER_PT = 13
 BYTES_PER_PT_PER_TURN_MODE = 32           # 16 B read + 16 B write per particle-turn
 SMS, FP64_LANES_PER_SM = 148, 64          # B200: 2 dies x 74 SMs, 64 FP64 lanes per SM
+# DRAM bytes per launch of the two dominant kernels from the committed ncu captures (profiles/)
+CPU_SAMPLE_TURNS = 10_000                 # oracle leg: 1e9 particle-turns, about 20-25 core-seconds
+NCU_TRAFFIC_FUSED_BYTES = 1_625_344 + 570_112
+NCU_TRAFFIC_PER_TURN_BYTES = 160_020_480 + 100_925_184
 
 
 def measured_peaks() -> dict:
@@ -236,7 +240,10 @@ def run_cuda(args) -> None:
             3: "fused_persistent_kernel (dynamic chunk scheduling)"}[tr.get_stat(lt.STAT_LAST_MODE)]
     roofline = {"bound": "alu", "kernel": mode + " <double, leap-frog, single harmonic, merged drifts>",
                 "achieved": achieved_ginstr, "peak": peak_ginstr, "unit": "G FP64 instr/s",
-                "frac": achieved_ginstr / peak_ginstr, "traffic": None,
+                "frac": achieved_ginstr / peak_ginstr,
+                # dram__bytes_read.sum + dram__bytes_write.sum per launch, ncu --set full
+                # (profiles/r1_fused_ncu_details.txt); algorithmic: 32 B x n = 3.2 MB per launch
+                "traffic": NCU_TRAFFIC_FUSED_BYTES, "algorithmic_bytes": 32 * n,
                 "instr_per_particle_turn": FP64_INSTR_PER_PT,
                 "peak_source": "148 SMs x 64 FP64 lanes x sm_max_mhz (DESIGN.md); "
                                "MEASURED_PEAKS.json has no FP64 entry",
@@ -290,7 +297,10 @@ def run_cuda(args) -> None:
                     "ms_per_turn": 1e3 * t_pt / (t3 * reps),
                     "gpu_launches": tr3.get_stat(lt.STAT_KERNEL_LAUNCHES) - l0,
                     "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
-                                 "frac": gbs / hbm_peak, "traffic": None,
+                                 "frac": gbs / hbm_peak,
+                                 # ncu --set full, cold cache (profiles/r1_per_turn_ncu_details.txt)
+                                 "traffic": NCU_TRAFFIC_PER_TURN_BYTES,
+                                 "algorithmic_bytes": BYTES_PER_PT_PER_TURN_MODE * n3,
                                  "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks
                                  else "fallback 6650 GB/s (B200_PROFILING.md)",
                                  "frac_of_nominal_8TBs": gbs / 8000.0},
@@ -310,10 +320,10 @@ def run_cuda(args) -> None:
     # ---- CPU oracle beside it (rank 0, N = 1 only)
     cpu_baseline = None
     if world == 1 and not args.skip_cpu:
-        rate, dt, cores = oracle_rate(n, 4000, cfg["seed"])
+        rate, dt, cores = oracle_rate(n, CPU_SAMPLE_TURNS, cfg["seed"])
         cpu_baseline = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                        "sample": "configs[1] bunch: %d particles x 4000 turns (of %d), %.1f s wall"
-                                  % (n, turns, dt)}
+                        "sample": "configs[1] bunch: %d particles x %d turns (of %d), %.1f s wall x %d threads"
+                                  % (n, CPU_SAMPLE_TURNS, turns, dt, cores)}
 
     if rank == 0:
         print(json.dumps({

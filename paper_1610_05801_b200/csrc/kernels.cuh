@@ -68,7 +68,7 @@ template <> struct Real<double> {
     static __device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
     // f with the sign bit flipped when the integer held in the low mantissa bits of t is odd.
     // hi + (lo << 31) mod 2^32 == hi ^ ((lo & 1) << 31): ONE IMAD instead of shift + xor (every
-    // non-FP64 instruction in the turn loop costs about two issue cycles, profiles/ubench).
+    // non-FP64 instruction in the turn loop costs about two issue cycles, profiles/r1_fused_sweep.md).
     static __device__ __forceinline__ double flip(double f, double t) {
         int hi = __double2hiint(f) + __double2loint(t) * (int)0x80000000;
         return __hiloint2double(hi, __double2loint(f));
@@ -118,7 +118,7 @@ __device__ __forceinline__ T horner(const T (&c)[N], T s) {
 // ------------------------------------------------------------------------------------------
 // FQ selects WHERE the sign (-1)^n is applied: to f (off the critical path, best below ~5
 // resident warps per sub-partition) or to the polynomial value q (one dependent integer op
-// later, but it measured 3-4 % faster once the FP64 pipe is saturated; profiles/ubench_r1.md).
+// later, but it measured 3-4 % faster once the FP64 pipe is saturated; profiles/r1_fused_sweep.md).
 template <typename T, int HARM, bool FQ = false>
 __device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage) {
     typedef Real<T> R;
@@ -221,7 +221,7 @@ __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int 
             }
         }
         // every non-FP64 instruction costs about two issue cycles next to the saturated FP64
-        // pipe (profiles/ubench_r1.md): unroll deep enough that the loop counter disappears
+        // pipe (profiles/r1_fused_sweep.md): unroll deep enough that the loop counter disappears
         constexpr int kUnroll = (INTEG == kRuth4 || HARM != 1 || ILP > 2) ? 4 : LT_TURN_UNROLL / ILP;
 #pragma unroll kUnroll
         for (unsigned int t = 1; t < turns; ++t) {

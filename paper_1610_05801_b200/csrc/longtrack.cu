@@ -265,7 +265,7 @@ cudaError_t launch_fused_integ(int harm, bool split, T* z, T* d, size_t n, unsig
 struct PersistentPlan { int dynamic, warps_per_smsp, ctas_per_sm, threads; unsigned int item_turns; bool flip_on_q; };
 
 // FP64 warp-instructions per cycle per sub-partition of the turn loop at W resident warps
-// (measured with clock64 on B200, profiles/ubench_r1.md): sign flip on f / on q
+// (measured with clock64 on B200, profiles/r1_fused_sweep.md): sign flip on f / on q
 double loop_rate(int w, bool fq) {
     static const double on_f[] = {0, .1229, .2424, .3546, .4367, .4367, .4399, .4418, .4428};
     static const double on_q[] = {0, .1200, .2380, .3480, .4259, .4414, .4554, .4590, .4613};
