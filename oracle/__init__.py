@@ -18,7 +18,9 @@ from ctypes import (POINTER, Structure, c_double, c_int, c_size_t, c_ubyte, c_ul
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRC = [os.path.join(_HERE, f) for f in ("longtrack_oracle.c", "map.inc", "longtrack_oracle.h")]
+_C_FILES = ("longtrack_oracle.c", "next_oracle.c")
+_SRC = [os.path.join(_HERE, f) for f in _C_FILES + ("map.inc", "programme.inc",
+                                                     "longtrack_oracle.h", "next_oracle.h")]
 _LIB = os.path.join(_HERE, "liblongtrack_oracle.so")
 
 EULER_CROMER, LEAPFROG, RUTH4 = 0, 1, 2
@@ -53,7 +55,7 @@ def build(force: bool = False) -> str:
     """Compile the oracle with gcc (building the checker is not using it)."""
     newest = max(os.path.getmtime(s) for s in _SRC)
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
-        cmd = ["gcc", *CFLAGS, "-o", _LIB, _SRC[0], "-lm"]
+        cmd = ["gcc", *CFLAGS, "-o", _LIB, *_C_FILES, "-lm"]
         subprocess.run(cmd, check=True, cwd=_HERE)
     return _LIB
 
@@ -94,6 +96,21 @@ def lib():
         L.lto_bucket_mask.argtypes = [pp, dp, dp, c_size_t, POINTER(c_ubyte)]
         L.lto_bucket_mask.restype = None
         L.lto_num_threads.restype = c_int
+        ull = POINTER(c_ulonglong)
+        L.lto_track_programme.argtypes = [pp, dp, dp, c_size_t, c_ulonglong, dp, dp]
+        L.lto_track_programme.restype = None
+        L.lto_track_programme_ld.argtypes = [pp, c_void_p, c_void_p, c_size_t, c_ulonglong, dp, dp]
+        L.lto_track_programme_ld.restype = None
+        L.lto_track_programme_moments.argtypes = [pp, dp, dp, c_size_t, c_ulonglong, dp, dp, c_void_p]
+        L.lto_track_programme_moments.restype = None
+        L.lto_slice_histogram.argtypes = [dp, c_size_t, c_double, c_double, c_int, ull]
+        L.lto_slice_histogram.restype = None
+        L.lto_track_slices.argtypes = [pp, dp, dp, c_size_t, c_ulonglong, c_double, c_double,
+                                       c_int, ull]
+        L.lto_track_slices.restype = None
+        L.lto_track_transverse.argtypes = [pp, dp, c_int, dp, dp, dp, dp, dp, dp, c_size_t,
+                                           c_ulonglong]
+        L.lto_track_transverse.restype = None
         L.lto_set_num_threads.argtypes = [c_int]
         _lib = L
     return _lib
@@ -205,3 +222,76 @@ def num_threads() -> int:
 
 def set_num_threads(n: int) -> None:
     lib().lto_set_num_threads(int(n))
+
+
+# ------------------------------------------------------------------ SURVEY.md sec. 8(f) rows f2-f4
+def _copy(a):
+    return _f64(np.array(a, dtype=np.float64, copy=True).ravel())
+
+
+def track_programme(p: Params, z, delta, volt_scale, phase_off):
+    """f2: one turn per programme entry; returns new (z, delta)."""
+    z, zp = _copy(z)
+    d, dp_ = _copy(delta)
+    a, ap = _f64(volt_scale)
+    s, sp = _f64(phase_off)
+    assert a.size == s.size
+    lib().lto_track_programme(ctypes.byref(p), zp, dp_, z.size, a.size, ap, sp)
+    return z, d
+
+
+def track_programme_ld(p: Params, z, delta, volt_scale, phase_off):
+    z = np.ascontiguousarray(np.array(z, dtype=np.longdouble, copy=True).ravel())
+    d = np.ascontiguousarray(np.array(delta, dtype=np.longdouble, copy=True).ravel())
+    a, ap = _f64(volt_scale)
+    s, sp = _f64(phase_off)
+    assert a.size == s.size and z.dtype.itemsize == 16
+    lib().lto_track_programme_ld(ctypes.byref(p), z.ctypes.data, d.ctypes.data, z.size, a.size,
+                                 ap, sp)
+    return z, d
+
+
+def track_programme_moments(p: Params, z, delta, volt_scale, phase_off):
+    z, zp = _copy(z)
+    d, dp_ = _copy(delta)
+    a, ap = _f64(volt_scale)
+    s, sp = _f64(phase_off)
+    assert a.size == s.size
+    out = np.zeros(a.size, dtype=MOMENTS_DTYPE)
+    lib().lto_track_programme_moments(ctypes.byref(p), zp, dp_, z.size, a.size, ap, sp,
+                                      out.ctypes.data)
+    return z, d, out
+
+
+def slice_histogram(z, z_lo: float, z_hi: float, n_slices: int):
+    """f4: uint64[n_slices + 2] = [below, slices..., above]."""
+    z, zp = _f64(z)
+    h = np.zeros(n_slices + 2, dtype=np.uint64)
+    lib().lto_slice_histogram(zp, z.size, float(z_lo), float(z_hi), int(n_slices),
+                              h.ctypes.data_as(POINTER(c_ulonglong)))
+    return h
+
+
+def track_slices(p: Params, z, delta, turns: int, z_lo: float, z_hi: float, n_slices: int):
+    z, zp = _copy(z)
+    d, dp_ = _copy(delta)
+    h = np.zeros((int(turns), n_slices + 2), dtype=np.uint64)
+    lib().lto_track_slices(ctypes.byref(p), zp, dp_, z.size, int(turns), float(z_lo),
+                           float(z_hi), int(n_slices), h.ctypes.data_as(POINTER(c_ulonglong)))
+    return z, d, h
+
+
+def track_transverse(p: Params, matrices, x, xp, y, yp, z, delta, turns: int):
+    """f3: matrices = array [n_seg, 4, 4]; returns new (x, xp, y, yp, z, delta); z/delta may be None."""
+    m, mp = _f64(np.asarray(matrices, dtype=np.float64).reshape(-1, 16))
+    arrs = [_copy(a) for a in (x, xp, y, yp)]
+    n = arrs[0][0].size
+    if z is None:
+        zz = dd = None
+        zp = dp_ = None
+    else:
+        zz, zp = _copy(z)
+        dd, dp_ = _copy(delta)
+    lib().lto_track_transverse(ctypes.byref(p), mp, m.shape[0], arrs[0][1], arrs[1][1], arrs[2][1],
+                               arrs[3][1], zp, dp_, n, int(turns))
+    return tuple(a for a, _ in arrs) + (zz, dd)
