@@ -213,6 +213,72 @@ int lt_moments_from_sums(const lt_sums *sums_host, size_t count, lt_moments *out
 int lt_track_fused_host(lt_tracker *tr, double *z_host, double *delta_host, size_t n,
                         unsigned long long turns, unsigned long long *count_host);
 
+/* ========================================================================================
+ * Rows SURVEY.md sec. 8(f) marks "next" (fp64 only).  The paper prints no formula for any of
+ * them; the readings are DESIGN.md G28-G30.
+ * ======================================================================================== */
+
+/* -- f2: turn-dependent RF programme (sec. 2.2: the "parameter changes of the
+ *    accelerator setting (as in the above hollow bunch setting)" that the paper's C/CUDA
+ *    extraction left out; G28) ----------------------------------------------------
+ * volt_scale_dev[t], phase_off_dev[t] (device, `turns` doubles each; t = 0-based) apply to
+ * EVERY kick of turn t+1 (Ruth4: all three sub-kicks):
+ *     F_t(z) = a_t A [ sin(phi_s + kappa z + psi_t) - sin(phi_s) + r sin(2 (kappa z + psi_t)) ]
+ * a_t = volt_scale[t] = V_t / V (dimensionless), psi_t = phase_off[t] [rad].  a_t = 1, psi_t = 0
+ * is the plain map.  The tables are read while the call's work runs: keep them unchanged until
+ * the stream has been synchronised.  lt_track_programme is the fused multi-turn mode (state in
+ * registers, FP64-pipe bound, 15 instead of 13 FP64 instructions per particle-turn);
+ * lt_track_programme_per_turn is the per-turn mode with the same outputs as lt_track_per_turn. */
+int lt_track_programme(lt_tracker *tr, double *z_dev, double *delta_dev, size_t n,
+                       unsigned long long turns, const double *volt_scale_dev,
+                       const double *phase_off_dev, void *stream);
+int lt_track_programme_per_turn(lt_tracker *tr, double *z_dev, double *delta_dev, size_t n,
+                                unsigned long long turns, const double *volt_scale_dev,
+                                const double *phase_off_dev, lt_moments *moments_dev,
+                                lt_sums *sums_dev, void *stream);
+
+/* -- f4: longitudinal slicing at the interaction point (sec. 1.1: "the fields of
+ *    the particle distribution are constructed"; the memory-bound regime;
+ *    DESIGN.md G29) ---------------------------------------------------------------------------
+ * Uniform slices of z over [z_lo, z_hi), inv = n_slices / (z_hi - z_lo) in fp64:
+ *     z < z_lo        -> hist[0]             ("below")
+ *     not (z < z_hi)  -> hist[n_slices + 1]  ("above"; NaN lands here)
+ *     otherwise          u = (z - z_lo) * inv (two roundings, no FMA); s = floor(u) clamped to
+ *                        n_slices - 1;  hist[1 + s]
+ * hist_dev has n_slices + 2 counters (unsigned 64-bit) per histogram and is OVERWRITTEN.
+ * Requires z_lo < z_hi (finite) and 1 <= n_slices <= 2^20, else LT_E_PARAM.
+ * lt_slice_histogram: histogram of a given state.  lt_track_slices: per-turn mode -- one launch
+ * per turn tracks the turn and, in the same pass over HBM, fills hist_dev[t * (n_slices + 2) ..]
+ * with the histogram of z AFTER turn t+1 (t = 0 .. turns-1); moments_dev / sums_dev as in
+ * lt_track_per_turn, or NULL. */
+int lt_slice_histogram(lt_tracker *tr, const double *z_dev, size_t n, double z_lo, double z_hi,
+                       int n_slices, unsigned long long *hist_dev, void *stream);
+int lt_track_slices(lt_tracker *tr, double *z_dev, double *delta_dev, size_t n,
+                    unsigned long long turns, double z_lo, double z_hi, int n_slices,
+                    unsigned long long *hist_dev, lt_moments *moments_dev, lt_sums *sums_dev,
+                    void *stream);
+
+/* -- f3: transverse plane (sec. 1.1.1: "linear transfer matrices, i.e. the same
+ *    matrix is repeatedly acting on the typically 10^5 to 10^7 macro-particles' state vectors";
+ *    Fig. 2: pushed "from one interaction point to another"; G30) --------
+ * lt_set_transverse: the lattice, n_seg (1..256) 4x4 matrices in HOST memory, ROW-MAJOR,
+ * matrices_host[16 s + 4 i + j] = (M_s)_ij; copied by the call (n_seg = 0 clears it).
+ * One turn = for s = 0 .. n_seg-1 in order: u <- M_s u with u = (x, x', y, y'), row i evaluated
+ * left to right, ((M_i0 x + M_i1 x') + M_i2 y) + M_i3 y' (the library uses FMAs in that order);
+ * then the longitudinal turn of (z, delta) by the tracker's map.  The planes are not coupled.
+ * x/xp/y/yp (and z/delta) are separate device arrays of n doubles, updated in place; z_dev and
+ * delta_dev may both be NULL (transverse plane only).  Without a lattice: LT_E_PARAM.
+ * _fused: `turns` turns with the state in registers (FP64-pipe bound, 16 FP64 instructions per
+ * segment and particle); _per_turn: one launch per turn, every coordinate through HBM (64 B per
+ * particle-turn, 96 B with the longitudinal plane; HBM bound). */
+int lt_set_transverse(lt_tracker *tr, const double *matrices_host, int n_seg);
+int lt_track_transverse_fused(lt_tracker *tr, double *x_dev, double *xp_dev, double *y_dev,
+                              double *yp_dev, double *z_dev, double *delta_dev, size_t n,
+                              unsigned long long turns, void *stream);
+int lt_track_transverse_per_turn(lt_tracker *tr, double *x_dev, double *xp_dev, double *y_dev,
+                                 double *yp_dev, double *z_dev, double *delta_dev, size_t n,
+                                 unsigned long long turns, void *stream);
+
 /* -- roofline probes (measurement only, not on the hot path) ------------------------------
  * Runs a dependent-chain DFMA kernel (`chains` independent chains per thread, `iters` FMAs
  * per chain) and returns achieved FP64 lane-instructions per second in *rate. Synchronises. */

@@ -16,12 +16,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblongtrack.so")
-SOURCES = [os.path.join(CSRC, "longtrack.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "sinpi_coeffs.h"),
+SOURCES = [os.path.join(CSRC, "longtrack.cu"), os.path.join(CSRC, "longtrack_next.cu")]
+DEPS = SOURCES + [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "kernels_next.cuh"),
+                  os.path.join(CSRC, "tracker.hpp"), os.path.join(CSRC, "sinpi_coeffs.h"),
                   os.path.join(ROOT, "include", "longtrack.h")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+              "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--threads", "2"]
 
 
 def nvcc() -> str:

@@ -119,15 +119,22 @@ __device__ __forceinline__ T horner(const T (&c)[N], T s) {
 // FQ selects WHERE the sign (-1)^n is applied: to f (off the critical path, best below ~5
 // resident warps per sub-partition) or to the polynomial value q (one dependent integer op
 // later, but it measured 3-4 % faster once the FP64 pipe is saturated; profiles/r1_fused_sweep.md).
-template <typename T, int HARM, bool FQ = false>
-__device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage) {
+// PROG (RF programme; G28): the kick of this turn is
+//     a * A [ sin(phi_s + pi (v + p)) - sin(phi_s) + r sin(2 pi (v + p)) ],
+// a = voltage scale, p = phase offset in half periods.  PROG = 1: add p here (fast path, the
+// state is v); PROG = 2: the caller already folded p into v (exact path: v = fma(z, kappa/pi, p)).
+template <typename T, int HARM, bool FQ = false, int PROG = 0>
+__device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage, T a = T(1),
+                                  T p = T(0)) {
     typedef Real<T> R;
     constexpr int NS = R::NS, NC = R::NC;
+    if (PROG == 1) v = R::add(v, p);
     if (HARM == 1) {
         T t;
         T f = reduce_half_periods(v, &t);
         T s = R::mul(f, f);
         T q = horner<T, NS>(P.sinA[stage], s);
+        if (PROG) q = R::mul(q, a);
         if (FQ) return R::fma(f, R::flip(q, t), delta);
         return R::fma(R::flip(f, t), q, delta);
     } else if (HARM == 2) {
@@ -136,6 +143,7 @@ __device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage
         T s = R::mul(f, f);
         T q = horner<T, NS>(P.sinA[stage], s);   // tau A sin(pi f)/f
         T c = horner<T, NC>(P.cos1, s);           // cos(pi f)
+        if (PROG) q = R::mul(q, a);
         // sin and cos both change sign with the parity of n: flip f, and flip 2r for the cos
         T m = R::fma(R::flip_by(P.two_r, t), c, T(1));
         if (FQ) return R::fma(f, R::flip(R::mul(q, m), t), delta);
@@ -150,7 +158,7 @@ __device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage
         T s2 = R::mul(f2, f2);
         T sn2 = R::mul(R::flip(f2, t2), horner<T, NS>(P.sin1, s2));
         acc = R::fma(P.r, sn2, acc);
-        return R::fma(P.kickA[stage], acc, delta);
+        return R::fma(PROG ? R::mul(P.kickA[stage], a) : P.kickA[stage], acc, delta);
     }
 }
 
@@ -158,42 +166,48 @@ __device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage
 // One full turn on the EXACT path: the state is z itself, every half drift is its own FMA
 // (bit-identical between the per-turn kernel, the split-drift fused kernel and any chunking).
 // ------------------------------------------------------------------------------------------
-template <typename T, int INTEG, int HARM>
-__device__ __forceinline__ void turn_exact(T& z, T& delta, const MapConsts<T>& P) {
+template <typename T, int INTEG, int HARM, bool PROG = false>
+__device__ __forceinline__ void turn_exact(T& z, T& delta, const MapConsts<T>& P, T a = T(1),
+                                           T p = T(0)) {
     typedef Real<T> R;
+    constexpr int PK = PROG ? 2 : 0;
+#define LT_PHASE(zz) (PROG ? R::fma(zz, P.to_phase, p) : R::mul(zz, P.to_phase))
     if (INTEG == kLeapfrog) {
         z = R::fma(-P.zdrift_lead, delta, z);
-        delta = kick<T, HARM>(R::mul(z, P.to_phase), delta, P, 0);
+        delta = kick<T, HARM, false, PK>(LT_PHASE(z), delta, P, 0, a);
         z = R::fma(-P.zdrift_trail, delta, z);
     } else if (INTEG == kEulerCromer) {
-        delta = kick<T, HARM>(R::mul(z, P.to_phase), delta, P, 0);
+        delta = kick<T, HARM, false, PK>(LT_PHASE(z), delta, P, 0, a);
         z = R::fma(-P.zdrift_trail, delta, z);
     } else {
         z = R::fma(-P.zdrift_lead, delta, z);
-        delta = kick<T, HARM>(R::mul(z, P.to_phase), delta, P, 0);
+        delta = kick<T, HARM, false, PK>(LT_PHASE(z), delta, P, 0, a);
         z = R::fma(-P.zdrift_mid, delta, z);
-        delta = kick<T, HARM>(R::mul(z, P.to_phase), delta, P, 1);
+        delta = kick<T, HARM, false, PK>(LT_PHASE(z), delta, P, 1, a);
         z = R::fma(-P.zdrift_mid, delta, z);
-        delta = kick<T, HARM>(R::mul(z, P.to_phase), delta, P, 2);
+        delta = kick<T, HARM, false, PK>(LT_PHASE(z), delta, P, 2, a);
         z = R::fma(-P.zdrift_trail, delta, z);
     }
+#undef LT_PHASE
 }
 
 // One turn on the FAST path, state = phase v, WITHOUT its leading drift and with the trailing
 // drift given by the caller (merged with the next turn's leading drift, or the plain trailing
 // one at the end of a call).
-template <typename T, int INTEG, int HARM, bool FQ = false>
-__device__ __forceinline__ void turn_fast(T& v, T& delta, const MapConsts<T>& P, T trailing) {
+template <typename T, int INTEG, int HARM, bool FQ = false, bool PROG = false>
+__device__ __forceinline__ void turn_fast(T& v, T& delta, const MapConsts<T>& P, T trailing,
+                                          T a = T(1), T p = T(0)) {
     typedef Real<T> R;
+    constexpr int PK = PROG ? 1 : 0;
     if (INTEG == kRuth4) {
-        delta = kick<T, HARM, FQ>(v, delta, P, 0);
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 0, a, p);
         v = R::fma(-P.drift_mid, delta, v);
-        delta = kick<T, HARM, FQ>(v, delta, P, 1);
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 1, a, p);
         v = R::fma(-P.drift_mid, delta, v);
-        delta = kick<T, HARM, FQ>(v, delta, P, 2);
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 2, a, p);
         v = R::fma(-trailing, delta, v);
     } else {
-        delta = kick<T, HARM, FQ>(v, delta, P, 0);
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 0, a, p);
         v = R::fma(-trailing, delta, v);
     }
 }
@@ -203,14 +217,19 @@ __device__ __forceinline__ void turn_fast(T& v, T& delta, const MapConsts<T>& P,
 // trailing drift and converts back, in between consecutive half drifts are merged.  Between
 // chunks of one call the z array therefore holds v mid-drift, which makes the result of a
 // call independent of how its turns are chunked.  SPLIT: exact path, state is z.
-template <typename T, int INTEG, int HARM, bool SPLIT, int ILP, bool FQ>
+// PROG: prog[k] = (a, p) of the k-th turn of this call to advance (voltage scale, phase offset
+// in half periods; one uniform 16-byte load per turn and warp).
+template <typename T, int INTEG, int HARM, bool SPLIT, int ILP, bool FQ, bool PROG = false>
 __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int turns, int first,
-                                        int last, const MapConsts<T>& P) {
+                                        int last, const MapConsts<T>& P,
+                                        const double2* __restrict__ prog = nullptr) {
     typedef Real<T> R;
     if (SPLIT) {
         for (unsigned int t = 0; t < turns; ++t) {
+            T a = T(1), p = T(0);
+            if (PROG) { const double2 e = __ldg(prog + t); a = (T)e.x; p = (T)e.y; }
 #pragma unroll
-            for (int j = 0; j < ILP; ++j) turn_exact<T, INTEG, HARM>(x[j], dl[j], P);
+            for (int j = 0; j < ILP; ++j) turn_exact<T, INTEG, HARM, PROG>(x[j], dl[j], P, a, p);
         }
     } else {
         if (first) {
@@ -225,14 +244,18 @@ __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int 
         constexpr int kUnroll = (INTEG == kRuth4 || HARM != 1 || ILP > 2) ? 4 : LT_TURN_UNROLL / ILP;
 #pragma unroll kUnroll
         for (unsigned int t = 1; t < turns; ++t) {
+            T a = T(1), p = T(0);
+            if (PROG) { const double2 e = __ldg(prog + (t - 1)); a = (T)e.x; p = (T)e.y; }
 #pragma unroll
             for (int j = 0; j < ILP; ++j)
-                turn_fast<T, INTEG, HARM, FQ>(x[j], dl[j], P, P.drift_merged);
+                turn_fast<T, INTEG, HARM, FQ, PROG>(x[j], dl[j], P, P.drift_merged, a, p);
         }
         const T trailing = last ? P.drift_trail : P.drift_merged;
+        T a = T(1), p = T(0);
+        if (PROG) { const double2 e = __ldg(prog + (turns - 1)); a = (T)e.x; p = (T)e.y; }
 #pragma unroll
         for (int j = 0; j < ILP; ++j) {
-            turn_fast<T, INTEG, HARM, FQ>(x[j], dl[j], P, trailing);
+            turn_fast<T, INTEG, HARM, FQ, PROG>(x[j], dl[j], P, trailing, a, p);
             if (last) x[j] = R::mul(x[j], P.from_phase);
         }
     }
@@ -328,12 +351,14 @@ __device__ __forceinline__ void st_release_u32(unsigned int* p, unsigned int v) 
     asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ>
+// PROG: prog[k] = (a, p) of the k-th turn of THIS launch (RF programme, f2).
+template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ, bool PROG = false>
 __global__ void __launch_bounds__(1024, 1)
 fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, unsigned int turns,
                         unsigned int item_turns, int first_launch, int last_launch, int dynamic,
                         unsigned long long* __restrict__ ticket, unsigned int* __restrict__ done,
-                        const __grid_constant__ MapConsts<T> P) {
+                        const __grid_constant__ MapConsts<T> P,
+                        const double2* __restrict__ prog = nullptr) {
     extern __shared__ unsigned char residency_cap[];   // unused: sized to cap CTAs per SM
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned long long groups = (n + 31) / 32;
@@ -364,7 +389,8 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
         const int first = first_launch && c == 0;
         const int last = last_launch && c == nchunks - 1;
         const unsigned int nt = (c == nchunks - 1) ? turns - c * item_turns : item_turns;
-        advance<T, INTEG, HARM, SPLIT, 1, FQ>(x, dl, nt, first, last, P);
+        advance<T, INTEG, HARM, SPLIT, 1, FQ, PROG>(x, dl, nt, first, last, P,
+                                                    PROG ? prog + (size_t)c * item_turns : nullptr);
         if (i < n) { __stcg(z_arr + i, x[0]); __stcg(d_arr + i, dl[0]); }
         if (nchunks > 1) {
             __threadfence();
@@ -540,7 +566,7 @@ __device__ __forceinline__ MomentsOut moments_from(const SumsOut& s) {
     return m;
 }
 
-__global__ void finalize_kernel(const double* __restrict__ partials, int nparts, size_t n,
+static __global__ void finalize_kernel(const double* __restrict__ partials, int nparts, size_t n,
                                 unsigned long long* __restrict__ cursor, unsigned int* done,
                                 MomentsOut* __restrict__ moments, SumsOut* __restrict__ sums,
                                 unsigned long long* __restrict__ count_out) {
@@ -582,7 +608,7 @@ __global__ void finalize_kernel(const double* __restrict__ partials, int nparts,
     }
 }
 
-__global__ void set_cursor_kernel(unsigned long long* cursor, unsigned int* done,
+static __global__ void set_cursor_kernel(unsigned long long* cursor, unsigned int* done,
                                   unsigned long long value) {
     *cursor = value;
     *done = 0u;

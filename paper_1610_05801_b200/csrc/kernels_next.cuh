@@ -1,0 +1,381 @@
+// kernels_next.cuh -- sm_100a device code for the rows SURVEY.md sec. 8(f) marks "next":
+//   f2  turn-dependent RF programme in per-turn mode      (PAPER.md:76;  DESIGN.md G28)
+//       (its fused-mode form is the PROG option of kernels.cuh's persistent kernel)
+//   f4  longitudinal slicing fused into the per-turn pass  (G29)
+//   f3  transverse linear transfer maps                    (Fig. 2; G30)
+// CUDA path only: shares nothing with oracle/.
+#pragma once
+
+#include "kernels.cuh"
+
+namespace lt {
+
+// ------------------------------------------------------------------------------------------
+// f4: slice index of one particle (reading G29).  The decision is taken exactly as stated --
+// one subtraction, one multiplication by inv = S/(z_hi - z_lo), each rounded once, no FMA --
+// so that for the same z every implementation lands in the same slice.
+//   0: z < z_lo ("below")    S+1: not (z < z_hi) ("above", NaN included)    1+s otherwise
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int slice_bin(double z, double z_lo, double z_hi, double inv, int S) {
+    if (z < z_lo) return 0;
+    if (!(z < z_hi)) return S + 1;
+    const double u = __dmul_rn(__dsub_rn(z, z_lo), inv);   // >= 0: truncation is floor
+    const int s = (int)u;
+    return 1 + (s < S - 1 ? s : S - 1);
+}
+
+// What the per-turn kernel needs beyond the plain map; every field is uniform over the grid.
+struct TurnExtras {
+    const double* volt_scale;            // [turns] a_t or nullptr (device)
+    const double* phase_off;             // [turns] psi_t in rad or nullptr (device)
+    const unsigned long long* cursor;    // absolute index of the batch's first turn (device)
+    int k;                               // this launch's turn within the batch
+    double inv_pi;
+    unsigned long long* hist;            // [turns][S+2] or nullptr (device), zeroed by the caller
+    double z_lo, z_hi, inv;
+    int n_slices;
+    int replicas;                        // shared-memory copies of the histogram; 0 = global atomics
+};
+
+// CTA-private histogram in shared memory, `replicas` copies indexed by lane so that the
+// particles of one warp that fall into the same slice do not serialise on one address.
+struct SliceAcc {
+    unsigned int* sh;
+    unsigned long long* out;
+    double z_lo, z_hi, inv;
+    int S, stride, rep_mask;
+    __device__ __forceinline__ void init(const TurnExtras& X, unsigned long long turn,
+                                         unsigned int* smem) {
+        sh = smem; S = X.n_slices; stride = S + 2; rep_mask = X.replicas - 1;
+        z_lo = X.z_lo; z_hi = X.z_hi; inv = X.inv;
+        out = X.hist + turn * (unsigned long long)stride;
+        if (X.replicas > 0) {
+            for (int i = threadIdx.x; i < X.replicas * stride; i += blockDim.x) sh[i] = 0u;
+            __syncthreads();
+        }
+    }
+    __device__ __forceinline__ void add(double z) {
+        const int b = slice_bin(z, z_lo, z_hi, inv, S);
+        if (rep_mask >= 0) atomicAdd(sh + ((int)(threadIdx.x & 31u) & rep_mask) * stride + b, 1u);
+        else atomicAdd(out + b, 1ULL);
+    }
+    __device__ __forceinline__ void flush() {
+        if (rep_mask < 0) return;
+        __syncthreads();
+        for (int b = threadIdx.x; b < stride; b += blockDim.x) {
+            unsigned int c = 0u;
+            for (int r = 0; r <= rep_mask; ++r) c += sh[r * stride + b];
+            if (c) atomicAdd(out + b, (unsigned long long)c);
+        }
+    }
+};
+
+// ------------------------------------------------------------------------------------------
+// Per-turn kernel with the f2 / f4 extras: the structure of per_turn_kernel (persistent CTAs,
+// double2 tiles, all loads of a tile before its arithmetic, moments fused), plus
+//   - the turn's programme entry (a_t, psi_t/pi), read once per CTA from the device tables at
+//     index *cursor + k (the cursor lives on the device so one CUDA graph serves every batch);
+//   - the slice histogram of z after the turn, in shared memory, flushed with one 64-bit
+//     atomic per non-empty slice and CTA (integer adds: the result is order-independent).
+// Still 32 B of HBM traffic per particle-turn.
+// ------------------------------------------------------------------------------------------
+template <int INTEG, int HARM, bool MOMENTS, int UNR>
+__global__ void per_turn_extra_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr,
+                                      size_t n, int reverse, double* __restrict__ partials,
+                                      const __grid_constant__ MapConsts<double> P,
+                                      const __grid_constant__ TurnExtras X) {
+    extern __shared__ unsigned int slice_smem[];
+    const unsigned long long turn = *X.cursor + (unsigned long long)X.k;
+    const bool prog = X.volt_scale != nullptr;
+    const bool slices = X.hist != nullptr;
+    double a = 1.0, p = 0.0;
+    if (prog) {
+        a = __ldg(X.volt_scale + turn);
+        p = __dmul_rn(__ldg(X.phase_off + turn), X.inv_pi);
+    }
+    SliceAcc sl;
+    if (slices) sl.init(X, turn, slice_smem);
+    Sums acc;
+    acc.zero();
+    const size_t npair = n >> 1;
+    const size_t tile_pairs = (size_t)blockDim.x * UNR;
+    const size_t ntiles = (npair + tile_pairs - 1) / tile_pairs;
+    for (size_t tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
+        const size_t tix = reverse ? (ntiles - 1 - tl) : tl;
+        const size_t base = tix * tile_pairs;
+        double2 zz[UNR], dd[UNR];
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            size_t q = base + (size_t)u * blockDim.x + threadIdx.x;
+            if (q < npair) {
+                zz[u] = reinterpret_cast<const double2*>(z_arr)[q];
+                dd[u] = reinterpret_cast<const double2*>(d_arr)[q];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) {
+            size_t q = base + (size_t)u * blockDim.x + threadIdx.x;
+            if (q < npair) {
+                if (prog) {
+                    turn_exact<double, INTEG, HARM, true>(zz[u].x, dd[u].x, P, a, p);
+                    turn_exact<double, INTEG, HARM, true>(zz[u].y, dd[u].y, P, a, p);
+                } else {
+                    turn_exact<double, INTEG, HARM>(zz[u].x, dd[u].x, P);
+                    turn_exact<double, INTEG, HARM>(zz[u].y, dd[u].y, P);
+                }
+                reinterpret_cast<double2*>(z_arr)[q] = zz[u];
+                reinterpret_cast<double2*>(d_arr)[q] = dd[u];
+                if (MOMENTS) {
+                    acc.add(zz[u].x, dd[u].x, in_bucket<double>(zz[u].x, dd[u].x, P));
+                    acc.add(zz[u].y, dd[u].y, in_bucket<double>(zz[u].y, dd[u].y, P));
+                }
+                if (slices) { sl.add(zz[u].x); sl.add(zz[u].y); }
+            }
+        }
+    }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        double z1 = z_arr[n - 1], d1 = d_arr[n - 1];
+        if (prog) turn_exact<double, INTEG, HARM, true>(z1, d1, P, a, p);
+        else turn_exact<double, INTEG, HARM>(z1, d1, P);
+        z_arr[n - 1] = z1; d_arr[n - 1] = d1;
+        if (MOMENTS) acc.add(z1, d1, in_bucket<double>(z1, d1, P));
+        if (slices) sl.add(z1);
+    }
+    if (slices) sl.flush();
+    if (MOMENTS) block_reduce_store(acc, partials + (size_t)blockIdx.x * kPartialStride);
+}
+
+// scalar variant for arrays that are not 16-byte aligned (moments decided at run time)
+template <int INTEG, int HARM>
+__global__ void per_turn_extra_kernel_scalar(double* __restrict__ z_arr, double* __restrict__ d_arr,
+                                             size_t n, int moments, double* __restrict__ partials,
+                                             const __grid_constant__ MapConsts<double> P,
+                                             const __grid_constant__ TurnExtras X) {
+    extern __shared__ unsigned int slice_smem[];
+    const unsigned long long turn = *X.cursor + (unsigned long long)X.k;
+    const bool prog = X.volt_scale != nullptr;
+    const bool slices = X.hist != nullptr;
+    double a = 1.0, p = 0.0;
+    if (prog) {
+        a = __ldg(X.volt_scale + turn);
+        p = __dmul_rn(__ldg(X.phase_off + turn), X.inv_pi);
+    }
+    SliceAcc sl;
+    if (slices) sl.init(X, turn, slice_smem);
+    Sums acc;
+    acc.zero();
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (size_t)gridDim.x * blockDim.x) {
+        double z1 = z_arr[i], d1 = d_arr[i];
+        if (prog) turn_exact<double, INTEG, HARM, true>(z1, d1, P, a, p);
+        else turn_exact<double, INTEG, HARM>(z1, d1, P);
+        z_arr[i] = z1; d_arr[i] = d1;
+        if (moments) acc.add(z1, d1, in_bucket<double>(z1, d1, P));
+        if (slices) sl.add(z1);
+    }
+    if (slices) sl.flush();
+    if (moments) block_reduce_store(acc, partials + (size_t)blockIdx.x * kPartialStride);
+}
+
+// Advances the device turn cursor when a batch has no finalize launch to do it.
+static __global__ void advance_cursor_kernel(unsigned long long* cursor, unsigned long long by) {
+    *cursor += by;
+}
+
+// Histogram of a given state (lt_slice_histogram): grid-stride read of z only (8 B per particle).
+static __global__ void slice_histogram_kernel(const double* __restrict__ z_arr, size_t n,
+                                       const __grid_constant__ TurnExtras X) {
+    extern __shared__ unsigned int slice_smem[];
+    SliceAcc sl;
+    sl.init(X, 0ULL, slice_smem);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (size_t)gridDim.x * blockDim.x)
+        sl.add(z_arr[i]);
+    sl.flush();
+}
+
+// Programme tables for the fused kernel: (a_t, psi_t / pi) packed as double2.
+static __global__ void programme_pack_kernel(const double* __restrict__ volt_scale,
+                                      const double* __restrict__ phase_off, unsigned int count,
+                                      double inv_pi, double2* __restrict__ out) {
+    const unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < count) out[i] = make_double2(volt_scale[i], __dmul_rn(phase_off[i], inv_pi));
+}
+
+// ------------------------------------------------------------------------------------------
+// f3: transverse plane.  One turn = for every segment s in order  u <- M_s u,  u = (x, x', y, y'),
+// M_s row-major; row i is  fma(M_i3, y', fma(M_i2, y, fma(M_i1, x', M_i0 * x)))  -- the
+// association order of the definition, 16 FP64 instructions per segment and particle.
+// Up to kSegInParam matrices ride in the kernel-parameter constant bank and feed DFMA as direct
+// operands; longer lattices are read from global memory (uniform loads).
+// ------------------------------------------------------------------------------------------
+constexpr int kSegInParam = 4;
+struct TransConsts { double M[kSegInParam][16]; };
+
+__device__ __forceinline__ void apply_matrix(double (&u)[4], const double* __restrict__ M) {
+    double w[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        double acc = __dmul_rn(M[4 * i], u[0]);
+        acc = __fma_rn(M[4 * i + 1], u[1], acc);
+        acc = __fma_rn(M[4 * i + 2], u[2], acc);
+        w[i] = __fma_rn(M[4 * i + 3], u[3], acc);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) u[i] = w[i];
+}
+
+template <int NSEG>
+__device__ __forceinline__ void transverse_turn(double (&u)[4], const TransConsts& Q,
+                                                const double* __restrict__ Mg, int n_seg) {
+    if (NSEG > 0) {
+#pragma unroll
+        for (int s = 0; s < NSEG; ++s) apply_matrix(u, Q.M[s]);
+    } else {
+        for (int s = 0; s < n_seg; ++s) {
+            double M[16];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                const double2 e = __ldg(reinterpret_cast<const double2*>(Mg + 16 * (size_t)s) + k);
+                M[2 * k] = e.x; M[2 * k + 1] = e.y;
+            }
+            apply_matrix(u, M);
+        }
+    }
+}
+
+// Fused multi-turn transverse kernel: the persistent, ticketed work queue of
+// fused_persistent_kernel (items = chunk of item_turns turns x group of 32 particles) with the
+// four transverse coordinates -- and, when LONGI, the leap-frog single-harmonic longitudinal
+// turn of the same particle (fast path: phase state, merged drifts) -- held in registers.
+template <int NSEG, bool LONGI>
+__global__ void __launch_bounds__(1024, 1)
+transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp_arr,
+                             double* __restrict__ y_arr, double* __restrict__ yp_arr,
+                             double* __restrict__ z_arr, double* __restrict__ d_arr, size_t n,
+                             unsigned int turns, unsigned int item_turns, int first_launch,
+                             int last_launch, int dynamic, unsigned long long* __restrict__ ticket,
+                             unsigned int* __restrict__ done, const double* __restrict__ Mg,
+                             int n_seg, const __grid_constant__ TransConsts Q,
+                             const __grid_constant__ MapConsts<double> P) {
+    extern __shared__ unsigned char residency_cap[];   // unused: sized to cap CTAs per SM
+    const unsigned int lane = threadIdx.x & 31u;
+    const unsigned long long groups = (n + 31) / 32;
+    const unsigned int nchunks = (turns + item_turns - 1) / item_turns;
+    const unsigned long long total = groups * nchunks;
+    const unsigned long long slots = (unsigned long long)gridDim.x * (blockDim.x >> 5);
+    unsigned long long next = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
+    for (;;) {
+        unsigned long long t = next;
+        if (dynamic) {
+            if (lane == 0) t = atomicAdd(ticket, 1ULL);
+            t = __shfl_sync(0xffffffffu, t, 0);
+        } else {
+            next += slots;
+        }
+        if (t >= total) break;
+        const unsigned int c = (unsigned int)(t / groups);
+        const unsigned long long g = t - (unsigned long long)c * groups;
+        if (c > 0) {
+            while (ld_acquire_u32(done + g) < c) __nanosleep(64);
+        }
+        const size_t i = (size_t)g * 32 + lane;
+        const bool live = i < n;
+        double u[4], v = 0.0, dl = 0.0;
+        u[0] = live ? __ldcg(x_arr + i) : 0.0;
+        u[1] = live ? __ldcg(xp_arr + i) : 0.0;
+        u[2] = live ? __ldcg(y_arr + i) : 0.0;
+        u[3] = live ? __ldcg(yp_arr + i) : 0.0;
+        const int first = first_launch && c == 0;
+        const int last = last_launch && c == nchunks - 1;
+        const unsigned int nt = (c == nchunks - 1) ? turns - c * item_turns : item_turns;
+        if (LONGI) {
+            v = live ? __ldcg(z_arr + i) : 0.0;
+            dl = live ? __ldcg(d_arr + i) : 0.0;
+            if (first) v = __fma_rn(-P.drift_lead, dl, __dmul_rn(v, P.to_phase));
+        }
+#pragma unroll 2
+        for (unsigned int k = 1; k < nt; ++k) {
+            transverse_turn<NSEG>(u, Q, Mg, n_seg);
+            if (LONGI) turn_fast<double, kLeapfrog, 1, true>(v, dl, P, P.drift_merged);
+        }
+        transverse_turn<NSEG>(u, Q, Mg, n_seg);
+        if (LONGI) {
+            turn_fast<double, kLeapfrog, 1, true>(v, dl, P, last ? P.drift_trail : P.drift_merged);
+            if (last) v = __dmul_rn(v, P.from_phase);
+        }
+        if (live) {
+            __stcg(x_arr + i, u[0]); __stcg(xp_arr + i, u[1]);
+            __stcg(y_arr + i, u[2]); __stcg(yp_arr + i, u[3]);
+            if (LONGI) { __stcg(z_arr + i, v); __stcg(d_arr + i, dl); }
+        }
+        if (nchunks > 1) {
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) st_release_u32(done + g, c + 1);
+        }
+    }
+}
+
+// Per-turn transverse kernel: ONE turn per launch, all coordinates through HBM -- 64 B per
+// particle-turn for the transverse plane, 96 B with the longitudinal plane (LONGI: leap-frog,
+// single harmonic, exact path = bit-identical to per_turn_kernel).  The lattice (n_seg x 16
+// doubles) is staged in shared memory once per CTA.  VEC: every array is 16-byte aligned.
+template <bool LONGI, bool VEC>
+__global__ void transverse_per_turn_kernel(double* __restrict__ x_arr, double* __restrict__ xp_arr,
+                                           double* __restrict__ y_arr, double* __restrict__ yp_arr,
+                                           double* __restrict__ z_arr, double* __restrict__ d_arr,
+                                           size_t n, int reverse, const double* __restrict__ Mg,
+                                           int n_seg, const __grid_constant__ MapConsts<double> P) {
+    extern __shared__ double lattice[];
+    for (int k = threadIdx.x; k < 16 * n_seg; k += blockDim.x) lattice[k] = Mg[k];
+    __syncthreads();
+    if (VEC) {
+        const size_t npair = n >> 1;
+        const size_t ntiles = (npair + blockDim.x - 1) / blockDim.x;
+        for (size_t tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
+            const size_t tix = reverse ? (ntiles - 1 - tl) : tl;
+            const size_t q = tix * blockDim.x + threadIdx.x;
+            if (q >= npair) continue;
+            const double2 a0 = reinterpret_cast<const double2*>(x_arr)[q];
+            const double2 a1 = reinterpret_cast<const double2*>(xp_arr)[q];
+            const double2 a2 = reinterpret_cast<const double2*>(y_arr)[q];
+            const double2 a3 = reinterpret_cast<const double2*>(yp_arr)[q];
+            double2 zz, dd;
+            if (LONGI) {
+                zz = reinterpret_cast<const double2*>(z_arr)[q];
+                dd = reinterpret_cast<const double2*>(d_arr)[q];
+            }
+            double u[4] = {a0.x, a1.x, a2.x, a3.x}, w[4] = {a0.y, a1.y, a2.y, a3.y};
+            for (int s = 0; s < n_seg; ++s) {
+                apply_matrix(u, lattice + 16 * s);
+                apply_matrix(w, lattice + 16 * s);
+            }
+            reinterpret_cast<double2*>(x_arr)[q] = make_double2(u[0], w[0]);
+            reinterpret_cast<double2*>(xp_arr)[q] = make_double2(u[1], w[1]);
+            reinterpret_cast<double2*>(y_arr)[q] = make_double2(u[2], w[2]);
+            reinterpret_cast<double2*>(yp_arr)[q] = make_double2(u[3], w[3]);
+            if (LONGI) {
+                turn_exact<double, kLeapfrog, 1>(zz.x, dd.x, P);
+                turn_exact<double, kLeapfrog, 1>(zz.y, dd.y, P);
+                reinterpret_cast<double2*>(z_arr)[q] = zz;
+                reinterpret_cast<double2*>(d_arr)[q] = dd;
+            }
+        }
+    }
+    // scalar path: everything when !VEC, the odd last particle when VEC
+    const size_t i0 = VEC ? ((n & ~(size_t)1) + (size_t)blockIdx.x * blockDim.x + threadIdx.x)
+                          : ((size_t)blockIdx.x * blockDim.x + threadIdx.x);
+    for (size_t i = i0; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        double u[4] = {x_arr[i], xp_arr[i], y_arr[i], yp_arr[i]};
+        for (int s = 0; s < n_seg; ++s) apply_matrix(u, lattice + 16 * s);
+        x_arr[i] = u[0]; xp_arr[i] = u[1]; y_arr[i] = u[2]; yp_arr[i] = u[3];
+        if (LONGI) {
+            double z1 = z_arr[i], d1 = d_arr[i];
+            turn_exact<double, kLeapfrog, 1>(z1, d1, P);
+            z_arr[i] = z1; d_arr[i] = d1;
+        }
+    }
+}
+
+}  // namespace lt

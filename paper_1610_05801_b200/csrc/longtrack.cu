@@ -1,7 +1,7 @@
 // longtrack.cu -- host side of liblongtrack.so: the C ABI of include/longtrack.h, parameter
 // validation, derived constants, the launch planner and the kernel dispatch.
 // CUDA path only: nothing here includes, links or calls anything under oracle/.
-#include "../../include/longtrack.h"
+#include "tracker.hpp"
 
 #include <cmath>
 #include <cstdio>
@@ -9,73 +9,15 @@
 #include <cstring>
 #include <new>
 
-#include "kernels.cuh"
 #include "sinpi_coeffs.h"
 
 using namespace lt;
+using namespace lt_host;
 
 static_assert(sizeof(lt_sums) == sizeof(SumsOut) && sizeof(lt_sums) == 64, "lt_sums layout");
 static_assert(sizeof(lt_moments) == sizeof(MomentsOut) && sizeof(lt_moments) == 48, "lt_moments layout");
 
 namespace {
-
-constexpr int kBatchTurns = 64;          // per-turn launches per finalize launch / per graph
-constexpr int kPerTurnThreads = 256;
-constexpr int kPerTurnUnroll = 2;        // double2 pairs per thread per tile
-
-struct GraphKey {
-    void *z, *d, *moments, *sums;
-    size_t n;
-    int f32, reverse, grid;
-    bool operator==(const GraphKey& o) const {
-        return z == o.z && d == o.d && moments == o.moments && sums == o.sums && n == o.n &&
-               f32 == o.f32 && reverse == o.reverse && grid == o.grid;
-    }
-};
-
-}  // namespace
-
-struct lt_tracker {
-    lt_params p;
-    lt_derived_t g;
-    MapConsts<double> c64;
-    MapConsts<float> c32;
-    int harm;                 // 0 generic (phi_s != 0), 1 single, 2 double harmonic
-    // options
-    long long split_drifts, chunk_turns, fused_ilp, fused_block, per_turn_graph,
-        per_turn_ctas_per_sm, per_turn_reverse, fused_mode, item_turns, warps_per_smsp, flip_on_q;
-    // stats
-    long long launches, last_grid, last_block, last_ilp, last_mode, last_item_turns;
-    int sm_count;             // 0 until the first device call
-    int last_cuda_error;
-    // device scratch
-    double* partials;         // [kBatchTurns][grid][kPartialStride]
-    size_t partials_doubles;
-    unsigned long long* cursor;   // + done flag right behind it
-    unsigned long long* sched;    // persistent fused kernel: ticket, then done[groups] (u32)
-    size_t sched_bytes;
-    // host-buffer entry point
-    cudaStream_t own_stream;
-    double *stage_z, *stage_d;
-    unsigned long long* stage_count;
-    size_t stage_n;
-    // per-turn graph cache
-    cudaGraphExec_t graph_exec;
-    GraphKey graph_key;
-    cudaStream_t capture_stream;
-};
-
-namespace {
-
-#define LT_CUDA(tr, call)                                   \
-    do {                                                    \
-        cudaError_t e_ = (call);                            \
-        if (e_ != cudaSuccess) {                            \
-            (tr)->last_cuda_error = (int)e_;                \
-            (void)cudaGetLastError();                       \
-            return LT_E_CUDA;                               \
-        }                                                   \
-    } while (0)
 
 bool finite_all(const lt_params* p) {
     return std::isfinite(p->circumference_m) && std::isfinite(p->gamma) && std::isfinite(p->alpha_c) &&
@@ -159,6 +101,8 @@ void fill_consts(const lt_params* p, MapConsts<T>* c) {
     c->hn_delta = (T)(eta * C / (2.0L * (L)g.H_sep));
 }
 
+}  // namespace
+namespace lt_host {
 int ensure_device(lt_tracker* tr) {
     if (tr->sm_count > 0) return LT_OK;
     int dev = 0, sms = 0;
@@ -168,7 +112,11 @@ int ensure_device(lt_tracker* tr) {
     tr->sm_count = sms;
     return LT_OK;
 }
+}  // namespace lt_host
+namespace {
 
+}  // namespace
+namespace lt_host {
 int ensure_scratch(lt_tracker* tr, int grid) {
     const size_t need = (size_t)kBatchTurns * (size_t)grid * kPartialStride;
     if (tr->partials_doubles < need) {
@@ -184,8 +132,8 @@ int ensure_scratch(lt_tracker* tr, int grid) {
     }
     return LT_OK;
 }
-
-bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
+}  // namespace lt_host
+namespace {
 
 // ------------------------------------------------------------------------------------------
 // Launch planner for the fused kernel.  The whole ensemble should sit on the chip as ONE
@@ -262,8 +210,6 @@ cudaError_t launch_fused_integ(int harm, bool split, T* z, T* d, size_t n, unsig
 // pinned by a dummy dynamic shared-memory request so that the CTA scheduler cannot stack two on
 // one SM and leave another empty.
 // ------------------------------------------------------------------------------------------
-struct PersistentPlan { int dynamic, warps_per_smsp, ctas_per_sm, threads; unsigned int item_turns; bool flip_on_q; };
-
 // FP64 warp-instructions per cycle per sub-partition of the turn loop at W resident warps
 // (measured with clock64 on B200, profiles/r1_fused_sweep.md): sign flip on f / on q
 double loop_rate(int w, bool fq) {
@@ -273,6 +219,8 @@ double loop_rate(int w, bool fq) {
     return fq ? on_q[w] : on_f[w];
 }
 
+}  // namespace
+namespace lt_host {
 PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns) {
     const unsigned long long groups = (n + 31) / 32;
     const int sms = tr->sm_count;
@@ -323,6 +271,8 @@ PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long lon
     }
     return best;
 }
+}  // namespace lt_host
+namespace {
 
 template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ>
 cudaError_t launch_persistent_one(T* z, T* d, size_t n, unsigned int turns, unsigned int item_turns,
@@ -334,7 +284,7 @@ cudaError_t launch_persistent_one(T* z, T* d, size_t n, unsigned int turns, unsi
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     kern<<<sms * pl.ctas_per_sm, pl.threads, smem, st>>>(z, d, n, turns, item_turns, first, last, pl.dynamic, sched,
-                                      reinterpret_cast<unsigned int*>(sched + 1), c);
+                                      reinterpret_cast<unsigned int*>(sched + 1), c, nullptr);
     return cudaGetLastError();
 }
 
@@ -354,6 +304,8 @@ cudaError_t launch_persistent_integ(int harm, bool split, T* z, T* d, size_t n, 
 #undef LT_PK
 }
 
+}  // namespace
+namespace lt_host {
 int ensure_sched(lt_tracker* tr, size_t n) {
     const size_t groups = (n + 31) / 32;
     const size_t need = 8 + 4 * groups + 8;
@@ -364,6 +316,8 @@ int ensure_sched(lt_tracker* tr, size_t n) {
     }
     return LT_OK;
 }
+}  // namespace lt_host
+namespace {
 
 template <typename T>
 int track_fused_persistent(lt_tracker* tr, T* z, T* d, size_t n, unsigned long long turns,
@@ -482,6 +436,8 @@ cudaError_t launch_per_turn(const lt_tracker* tr, T* z, T* d, size_t n, int reve
 #undef LT_PT
 }
 
+}  // namespace
+namespace lt_host {
 int per_turn_grid(const lt_tracker* tr, size_t n) {
     const size_t tile = (size_t)kPerTurnThreads * kPerTurnUnroll * 2;
     size_t tiles = (n + tile - 1) / tile;
@@ -490,6 +446,8 @@ int per_turn_grid(const lt_tracker* tr, size_t n) {
     if (g < 1) g = 1;
     return (int)g;
 }
+}  // namespace lt_host
+namespace {
 
 // enqueue `nb` (<= kBatchTurns) turns starting at absolute turn index t0, then their finalize
 template <typename T>
@@ -542,7 +500,7 @@ int track_per_turn(lt_tracker* tr, T* z, T* d, size_t n, unsigned long long turn
     // full batches, replayed from a cached CUDA graph when enabled
     if (tr->per_turn_graph && turns >= 2ULL * kBatchTurns) {
         GraphKey key = {(void*)z, (void*)d, (void*)mo, (void*)so, n, sizeof(T) == 4,
-                        (int)tr->per_turn_reverse, grid};
+                        (int)tr->per_turn_reverse, grid, nullptr, nullptr, nullptr, 0.0, 0.0, 0};
         if (!tr->graph_exec || !(tr->graph_key == key)) {
             if (tr->graph_exec) { cudaGraphExecDestroy(tr->graph_exec); tr->graph_exec = nullptr; }
             if (!tr->capture_stream)
@@ -602,6 +560,18 @@ int state_sums(lt_tracker* tr, const T* z, const T* d, size_t n, lt_moments* mo,
 }
 
 }  // namespace
+
+namespace lt_host {
+int track_fused_f64(lt_tracker* tr, double* z, double* d, size_t n, unsigned long long turns,
+                    void* stream) {
+    return track_fused<double>(tr, z, d, n, turns, stream);
+}
+cudaError_t launch_per_turn_f64(const lt_tracker* tr, double* z, double* d, size_t n, int reverse,
+                                double* partials, bool moments, bool vec_ok, int grid,
+                                cudaStream_t st) {
+    return launch_per_turn<double>(tr, z, d, n, reverse, partials, moments, vec_ok, grid, tr->c64, st);
+}
+}  // namespace lt_host
 
 // ------------------------------------------------------------------------------------------
 // C ABI
@@ -667,6 +637,7 @@ int lt_destroy(lt_tracker* tr) {
     if (tr->stage_d) cudaFree(tr->stage_d);
     if (tr->stage_count) cudaFree(tr->stage_count);
     if (tr->own_stream) cudaStreamDestroy(tr->own_stream);
+    destroy_next(tr);
     (void)cudaGetLastError();
     delete tr;
     return LT_OK;

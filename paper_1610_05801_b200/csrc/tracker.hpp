@@ -1,0 +1,110 @@
+// tracker.hpp -- host-side internals shared by the translation units of liblongtrack.so
+// (longtrack.cu: the BASELINE path; longtrack_next.cu: SURVEY.md sec. 8(f) rows f2-f4).
+// Not part of the ABI.  CUDA path only: nothing here touches oracle/.
+#pragma once
+
+#include "../../include/longtrack.h"
+
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "kernels.cuh"
+
+namespace lt_host {
+
+constexpr int kBatchTurns = 64;          // per-turn launches per finalize launch / per graph
+constexpr int kPerTurnThreads = 256;
+constexpr int kPerTurnUnroll = 2;        // double2 pairs per thread per tile
+constexpr int kMaxSlices = 1 << 20;
+constexpr int kMaxSegments = 256;        // lattice staged in shared memory by the per-turn kernel
+
+struct GraphKey {
+    void *z, *d, *moments, *sums;
+    size_t n;
+    int f32, reverse, grid;
+    // extras (f2 / f4): tables, histogram and slicing grid baked into the captured launches
+    const void *volt, *phase;
+    void* hist;
+    double z_lo, z_hi;
+    int n_slices;
+    bool operator==(const GraphKey& o) const {
+        return z == o.z && d == o.d && moments == o.moments && sums == o.sums && n == o.n &&
+               f32 == o.f32 && reverse == o.reverse && grid == o.grid && volt == o.volt &&
+               phase == o.phase && hist == o.hist && z_lo == o.z_lo && z_hi == o.z_hi &&
+               n_slices == o.n_slices;
+    }
+};
+
+struct PersistentPlan {
+    int dynamic, warps_per_smsp, ctas_per_sm, threads;
+    unsigned int item_turns;
+    bool flip_on_q;
+};
+
+}  // namespace lt_host
+
+struct lt_tracker {
+    lt_params p;
+    lt_derived_t g;
+    lt::MapConsts<double> c64;
+    lt::MapConsts<float> c32;
+    int harm;                 // 0 generic (phi_s != 0), 1 single, 2 double harmonic
+    // options
+    long long split_drifts, chunk_turns, fused_ilp, fused_block, per_turn_graph,
+        per_turn_ctas_per_sm, per_turn_reverse, fused_mode, item_turns, warps_per_smsp, flip_on_q;
+    // stats
+    long long launches, last_grid, last_block, last_ilp, last_mode, last_item_turns;
+    int sm_count;             // 0 until the first device call
+    int last_cuda_error;
+    // device scratch
+    double* partials;         // [kBatchTurns][grid][kPartialStride]
+    size_t partials_doubles;
+    unsigned long long* cursor;   // + done flag right behind it
+    unsigned long long* sched;    // persistent fused kernel: ticket, then done[groups] (u32)
+    size_t sched_bytes;
+    // host-buffer entry point
+    cudaStream_t own_stream;
+    double *stage_z, *stage_d;
+    unsigned long long* stage_count;
+    size_t stage_n;
+    // per-turn graph cache
+    cudaGraphExec_t graph_exec;
+    lt_host::GraphKey graph_key;
+    cudaStream_t capture_stream;
+    // f2: packed programme table of the current fused chunk
+    double2* prog_table;
+    size_t prog_entries;
+    // f3: lattice
+    double* lattice_host;     // [n_seg][16], row-major
+    double* lattice_dev;
+    int n_seg, lattice_dirty;
+};
+
+#define LT_CUDA(tr, call)                                   \
+    do {                                                    \
+        cudaError_t e_ = (call);                            \
+        if (e_ != cudaSuccess) {                            \
+            (tr)->last_cuda_error = (int)e_;                \
+            (void)cudaGetLastError();                       \
+            return LT_E_CUDA;                               \
+        }                                                   \
+    } while (0)
+
+namespace lt_host {
+
+inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
+
+int ensure_device(lt_tracker* tr);
+int ensure_scratch(lt_tracker* tr, int grid);
+int ensure_sched(lt_tracker* tr, size_t n);
+PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns);
+int per_turn_grid(const lt_tracker* tr, size_t n);
+// the BASELINE path's fused / per-turn entry points, for calls that compose with them
+int track_fused_f64(lt_tracker* tr, double* z, double* d, size_t n, unsigned long long turns,
+                    void* stream);
+cudaError_t launch_per_turn_f64(const lt_tracker* tr, double* z, double* d, size_t n, int reverse,
+                                double* partials, bool moments, bool vec_ok, int grid,
+                                cudaStream_t st);
+void destroy_next(lt_tracker* tr);       // frees what longtrack_next.cu allocated
+
+}  // namespace lt_host

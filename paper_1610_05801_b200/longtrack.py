@@ -89,6 +89,15 @@ def _load():
         "lt_track_fused_host": (c_int, [vp, vp, vp, sz, ull, POINTER(ull)]),
         "lt_probe_fp64": (c_int, [c_int, c_int, c_int, c_longlong, POINTER(c_double),
                                   POINTER(c_double)]),
+        # SURVEY.md sec. 8(f) rows f2-f4
+        "lt_track_programme": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp]),
+        "lt_track_programme_per_turn": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp, vp, vp]),
+        "lt_slice_histogram": (c_int, [vp, vp, sz, c_double, c_double, c_int, vp, vp]),
+        "lt_track_slices": (c_int, [vp, vp, vp, sz, ull, c_double, c_double, c_int, vp, vp, vp,
+                                    vp]),
+        "lt_set_transverse": (c_int, [vp, vp, c_int]),
+        "lt_track_transverse_fused": (c_int, [vp, vp, vp, vp, vp, vp, vp, sz, ull, vp]),
+        "lt_track_transverse_per_turn": (c_int, [vp, vp, vp, vp, vp, vp, vp, sz, ull, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -187,6 +196,48 @@ class Tracker:
     def moments_now(self, z, delta, n: int, moments=None, sums=None, stream: int = 0):
         self._check(_lib.lt_moments_now(self._h, _ptr(z), _ptr(delta), n, _ptr(moments),
                                         _ptr(sums), stream))
+
+    # ---- SURVEY.md sec. 8(f) rows f2-f4 (device pointers; tables are device arrays too)
+    def track_programme(self, z, delta, n: int, turns: int, volt_scale, phase_off,
+                        stream: int = 0):
+        self._check(_lib.lt_track_programme(self._h, _ptr(z), _ptr(delta), n, turns,
+                                            _ptr(volt_scale), _ptr(phase_off), stream))
+
+    def track_programme_per_turn(self, z, delta, n: int, turns: int, volt_scale, phase_off,
+                                 moments=None, sums=None, stream: int = 0):
+        self._check(_lib.lt_track_programme_per_turn(self._h, _ptr(z), _ptr(delta), n, turns,
+                                                     _ptr(volt_scale), _ptr(phase_off),
+                                                     _ptr(moments), _ptr(sums), stream))
+
+    def slice_histogram(self, z, n: int, z_lo: float, z_hi: float, n_slices: int, hist,
+                        stream: int = 0):
+        self._check(_lib.lt_slice_histogram(self._h, _ptr(z), n, z_lo, z_hi, n_slices,
+                                            _ptr(hist), stream))
+
+    def track_slices(self, z, delta, n: int, turns: int, z_lo: float, z_hi: float,
+                     n_slices: int, hist, moments=None, sums=None, stream: int = 0):
+        self._check(_lib.lt_track_slices(self._h, _ptr(z), _ptr(delta), n, turns, z_lo, z_hi,
+                                         n_slices, _ptr(hist), _ptr(moments), _ptr(sums),
+                                         stream))
+
+    def set_transverse(self, matrices):
+        """matrices: numpy array [n_seg, 4, 4] (row-major) in host memory, or None to clear."""
+        if matrices is None:
+            self._check(_lib.lt_set_transverse(self._h, None, 0))
+            return
+        m = np.ascontiguousarray(matrices, dtype=np.float64).reshape(-1, 16)
+        self._check(_lib.lt_set_transverse(self._h, m.ctypes.data, m.shape[0]))
+
+    def track_transverse_fused(self, x, xp, y, yp, z, delta, n: int, turns: int,
+                               stream: int = 0):
+        self._check(_lib.lt_track_transverse_fused(self._h, _ptr(x), _ptr(xp), _ptr(y), _ptr(yp),
+                                                   _ptr(z), _ptr(delta), n, turns, stream))
+
+    def track_transverse_per_turn(self, x, xp, y, yp, z, delta, n: int, turns: int,
+                                  stream: int = 0):
+        self._check(_lib.lt_track_transverse_per_turn(self._h, _ptr(x), _ptr(xp), _ptr(y),
+                                                      _ptr(yp), _ptr(z), _ptr(delta), n, turns,
+                                                      stream))
 
     # ---- host-buffer call
     def track_fused_host(self, z_host, delta_host, n: int, turns: int, want_count: bool = False):

@@ -134,3 +134,98 @@ def shard_range(n: int, rank: int, world: int):
     base, extra = divmod(n, world)
     lo = rank * base + min(rank, extra)
     return lo, lo + base + (1 if rank < extra else 0)
+
+
+# ---------------------------------------------------------------------------------------------
+# Inputs for the rows SURVEY.md sec. 8(f) marks "next" (readings G28-G30).
+# Still input generation only: tables, matrices and coordinates are DATA handed to both sides.
+# ---------------------------------------------------------------------------------------------
+NEXT_CONFIGS = dict(
+    # f2: the shape of the paper's profiled hollow-bunch run (10^5 x 7*10^4) with the
+    # "parameter changes of the accelerator setting" switched on
+    f2_programme=dict(name="f2_programme", n=100_000, turns=70_000, integrator="leapfrog",
+                      ratio2=0.0, dist="gauss", sigma_z=0.23, seed=16110, programme_seed=16120),
+    # f3: "the same matrix is repeatedly acting on the typically 10^5 to 10^7 macro-particles'
+    # state vectors"
+    f3_transverse=dict(name="f3_transverse", n=1_000_000, turns=10_000, n_seg=4, seed=16111,
+                       lattice_seed=16121, sigma_z=0.23, per_turn_n=10_000_000, per_turn_turns=200),
+    # f4: slicing at the interaction point every turn, cfg3's shape (10^7 x 10^3)
+    f4_slices=dict(name="f4_slices", n=10_000_000, turns=1_000, n_slices=64, dist="gauss",
+                   sigma_z=0.23, seed=16112, ratio2=0.0),
+)
+
+
+def rf_programme(turns: int, seed: int, ring: dict = RING, ramp_to: float = 1.5,
+                 mod_amplitude: float = 0.05, mod_tune_ratio: float = 0.95,
+                 noise_rms: float = 1e-3):
+    """f2 input tables (volt_scale[turns], phase_off[turns]).
+
+    A hollow-bunch style manipulation (the paper gives no numbers for it):
+    the voltage ramps linearly from V to ramp_to*V over the run; the RF phase is modulated at
+    mod_tune_ratio * Q_s (near-resonant dipole excitation, which is how hollow bunches are
+    made) with a half-sine envelope over the first half of the run, plus seeded white RF phase
+    noise of noise_rms rad so that no two turns share a table entry."""
+    q = ring_numbers(ring)
+    t = np.arange(turns, dtype=np.float64)
+    a = 1.0 + (ramp_to - 1.0) * t / max(turns - 1, 1)
+    half = max(turns // 2, 1)
+    env = np.where(t < half, np.sin(np.pi * t / half), 0.0)
+    psi = mod_amplitude * env * np.sin(2.0 * np.pi * mod_tune_ratio * q["Qs"] * t)
+    psi = psi + np.random.default_rng(seed).normal(0.0, noise_rms, turns)
+    return np.ascontiguousarray(a), np.ascontiguousarray(psi)
+
+
+def twiss_transfer(a1: float, b1: float, a2: float, b2: float, phi: float):
+    """Courant-Snyder 2x2 transfer matrix from (alpha1, beta1) to (alpha2, beta2) with phase
+    advance phi (textbook form; these are INPUT matrices, not tracking arithmetic)."""
+    c, s = math.cos(phi), math.sin(phi)
+    r = math.sqrt(b2 / b1)
+    return np.array([[r * (c + a1 * s), math.sqrt(b1 * b2) * s],
+                     [-((1.0 + a1 * a2) * s + (a2 - a1) * c) / math.sqrt(b1 * b2),
+                      (c - a2 * s) / r]])
+
+
+def transverse_lattice(n_seg: int, seed: int, qx: float = 20.13, qy: float = 20.18,
+                       ring: dict = RING, coupling: float = 1e-4):
+    """f3 input: n_seg 4x4 segment matrices [n_seg, 4, 4] (row-major) for an SPS-like ring
+    (integer tunes 20, BASELINE's circumference).  Segment boundaries carry seeded Twiss
+    parameters around the smooth-approximation beta = R/Q; the phase advance is split evenly.
+    `coupling` adds a thin skew quadrupole (x' += k y, y' += k x) at the end of every segment so
+    that the off-diagonal 2x2 blocks are populated.  Returns (matrices, twiss_at_start) with
+    twiss_at_start = (alpha_x, beta_x, alpha_y, beta_y) for matching the bunch."""
+    rng = np.random.default_rng(seed)
+    R = ring["circumference_m"] / (2.0 * math.pi)
+    bx0, by0 = R / qx, R / qy
+    ax = rng.uniform(-1.0, 1.0, n_seg)
+    ay = rng.uniform(-1.0, 1.0, n_seg)
+    bx = bx0 * rng.uniform(0.6, 1.6, n_seg)
+    by = by0 * rng.uniform(0.6, 1.6, n_seg)
+    mats = np.zeros((n_seg, 4, 4))
+    for s in range(n_seg):
+        s2 = (s + 1) % n_seg
+        m = np.zeros((4, 4))
+        m[:2, :2] = twiss_transfer(ax[s], bx[s], ax[s2], bx[s2], 2.0 * math.pi * qx / n_seg)
+        m[2:, 2:] = twiss_transfer(ay[s], by[s], ay[s2], by[s2], 2.0 * math.pi * qy / n_seg)
+        skew = np.eye(4)
+        skew[1, 2] = coupling
+        skew[3, 0] = coupling
+        mats[s] = skew @ m
+    return np.ascontiguousarray(mats), (float(ax[0]), float(bx[0]), float(ay[0]), float(by[0]))
+
+
+def transverse_bunch(n: int, seed: int, twiss, eps_x: float = 8.0e-8, eps_y: float = 8.0e-8):
+    """f3 input: Gaussian (x, x', y, y') matched to `twiss` = (alpha_x, beta_x, alpha_y, beta_y)
+    with geometric emittances eps (SPS-like: 2 um normalised at gamma 27.7)."""
+    ax, bx, ay, by = twiss
+    g = np.random.default_rng(seed).normal(0.0, 1.0, (4, n))
+    x = math.sqrt(eps_x * bx) * g[0]
+    xp = math.sqrt(eps_x / bx) * (g[1] - ax * g[0])
+    y = math.sqrt(eps_y * by) * g[2]
+    yp = math.sqrt(eps_y / by) * (g[3] - ay * g[2])
+    return tuple(np.ascontiguousarray(v) for v in (x, xp, y, yp))
+
+
+def slice_grid(cfg: dict, ring: dict = RING):
+    """f4 input: the slicing interval = the RF bucket [-z_max, z_max), cfg['n_slices'] slices."""
+    q = ring_numbers(ring)
+    return -q["z_max"], q["z_max"], int(cfg["n_slices"])

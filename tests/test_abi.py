@@ -112,6 +112,53 @@ def test_no_cpu_fallback_device_calls_fail_loudly_without_a_gpu(lt):
     tr.track_fused(0, 0, 0, 10)
 
 
+def test_next_rows_validate_arguments_before_touching_a_device(lt):
+    """f2-f4 entry points: host-side checks (NULL, slicing grid, lattice) come first, so they
+    are testable without a GPU; with valid arguments and no GPU the calls fail with E_CUDA."""
+    import torch
+    from paper_1610_05801_b200 import workloads as wl
+    tr = lt.Tracker(wl.RING)
+
+    def code(fn, *args):
+        try:
+            fn(*args)
+        except lt.LongtrackError as e:
+            return e.code
+        return 0
+
+    buf = np.zeros(16)
+    # f4: slicing grid
+    for z_lo, z_hi, S in ((1.0, 1.0, 8), (1.0, -1.0, 8), (-1.0, 1.0, 0), (-1.0, 1.0, (1 << 20) + 1),
+                          (float("nan"), 1.0, 8), (-1.0, float("inf"), 8)):
+        assert code(tr.slice_histogram, buf, 8, z_lo, z_hi, S, buf) == lt.E_PARAM
+        assert code(tr.track_slices, buf, buf, 8, 4, z_lo, z_hi, S, buf) == lt.E_PARAM
+    assert code(tr.slice_histogram, buf, 8, -1.0, 1.0, 8, None) == lt.E_NULL
+    assert code(tr.track_slices, buf, buf, 8, 4, -1.0, 1.0, 8, None) == lt.E_NULL
+    assert code(tr.track_slices, buf, buf, 8, 0, -1.0, 1.0, 8, None) == 0      # zero turns: no-op
+    # f2: tables are required
+    assert code(tr.track_programme, buf, buf, 8, 4, None, buf) == lt.E_NULL
+    assert code(tr.track_programme_per_turn, buf, buf, 8, 4, buf, None) == lt.E_NULL
+    assert code(tr.track_programme, buf, buf, 0, 4, None, None) == 0           # n == 0: no-op
+    # f3: the lattice
+    four = (buf, buf, buf, buf)
+    assert code(tr.track_transverse_fused, *four, None, None, 8, 4) == lt.E_PARAM   # none set
+    bad = np.zeros((1, 4, 4))
+    bad[0, 2, 1] = np.inf
+    assert code(tr.set_transverse, bad) == lt.E_PARAM
+    assert code(tr.set_transverse, np.zeros((257, 4, 4))) == lt.E_PARAM
+    assert code(tr.set_transverse, np.eye(4)[None]) == 0
+    assert code(tr.track_transverse_fused, *four, buf, None, 8, 4) == lt.E_NULL     # z without delta
+    assert code(tr.track_transverse_per_turn, None, buf, buf, buf, None, None, 8, 4) == lt.E_NULL
+    assert code(tr.track_transverse_fused, *four, None, None, 0, 4) == 0
+    if not torch.cuda.is_available():
+        assert code(tr.track_transverse_fused, *four, None, None, 8, 4) == lt.E_CUDA
+        assert code(tr.track_programme, buf, buf, 8, 4, buf, buf) == lt.E_CUDA
+        assert code(tr.slice_histogram, buf, 8, -1.0, 1.0, 8, buf) == lt.E_CUDA
+        assert np.all(buf == 0.0)
+    assert code(tr.set_transverse, None) == 0
+    assert code(tr.track_transverse_fused, *four, None, None, 8, 4) == lt.E_PARAM
+
+
 def test_moments_from_sums_host_helper(lt):
     rng = np.random.default_rng(2)
     z, d = rng.normal(0.01, 0.2, 1000), rng.normal(0, 2e-3, 1000)
@@ -135,7 +182,8 @@ def test_product_path_never_touches_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
                 assert "longtrack_oracle" not in text and "lto_" not in text, f
-    for f in ("longtrack_oracle.c", "map.inc", "longtrack_oracle.h", "__init__.py"):
+    for f in ("longtrack_oracle.c", "map.inc", "longtrack_oracle.h", "__init__.py", "next_oracle.c",
+              "next_oracle.h", "programme.inc"):
         text = open(os.path.join(ROOT, "oracle", f)).read()
         assert "paper_1610_05801_b200" not in text.replace(
             "paper_1610_05801_b200/csrc/, include/longtrack.h", "").replace(
