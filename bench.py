@@ -163,6 +163,121 @@ def run_reference(args) -> None:
     }))
 
 
+
+# ----------------------------------------------------------------------------- next rows (f2-f4)
+def bench_next(lt, wl, torch, stream, peaks, peak_ginstr, max_over_ranks, world, rank):
+    """SURVEY.md sec. 8(f) rows f2 (RF programme, fused), f4 (per-turn + slicing histogram) and
+    f3 (transverse maps, fused and per-turn) at their NEXT_CONFIGS sizes, each against the
+    roofline that bounds it.  Device-timed with CUDA events."""
+    import numpy as np
+    sp = stream.cuda_stream
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def timed(fn, reps, restore=None):
+        t = 0.0
+        for r in range(reps + 1):                        # first repetition is the warm-up
+            if restore:
+                restore()
+            flush.fill_(r)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if r:
+                t += e0.elapsed_time(e1) * 1e-3
+        return max_over_ranks(t) / reps
+
+    def alu(instr, pts, sec):
+        g = instr * pts / sec / 1e9
+        return {"bound": "alu", "achieved": g, "peak": peak_ginstr, "unit": "G FP64 instr/s",
+                "frac": g / peak_ginstr, "instr_per_particle_turn": instr, "traffic": None}
+
+    def hbm(bytes_per_pt, pts, sec):
+        g = bytes_per_pt * pts / sec / 1e9
+        return {"bound": "hbm", "achieved": g, "peak": hbm_peak, "unit": "GB/s",
+                "frac": g / hbm_peak, "bytes_per_particle_turn": bytes_per_pt, "traffic": None}
+
+    out = {}
+    # f2: programme, fused mode, 15 FP64 instructions per particle-turn (13 + a_t scale + psi_t add)
+    c = wl.NEXT_CONFIGS["f2_programme"]
+    n, turns = c["n"], c["turns"]
+    z0, d0 = wl.gaussian_bunch(n, c["sigma_z"], c["seed"] + rank)
+    a, psi = wl.rf_programme(turns, c["programme_seed"])
+    z, d = torch.from_numpy(z0).cuda(), torch.from_numpy(d0).cuda()
+    zi, di = z.clone(), d.clone()
+    at, pt = torch.from_numpy(a).cuda(), torch.from_numpy(psi).cuda()
+    tr = lt.Tracker(wl.RING, "leapfrog")
+    sec = timed(lambda: tr.track_programme(z, d, n, turns, at, pt, sp), 5,
+                lambda: (z.copy_(zi), d.copy_(di)))
+    out["f2_programme_fused"] = {
+        "workload": "1e5 particles x 7e4 turns, per-turn (V_t, psi_t) tables, fused mode",
+        "value": world * n * turns / sec, "unit": UNIT, "ms": 1e3 * sec,
+        "roofline": alu(15, n * turns, sec)}
+    del z, d, zi, di, tr
+
+    # f4: per-turn mode + 64-slice histogram of z every turn (still 32 B per particle-turn)
+    c = wl.NEXT_CONFIGS["f4_slices"]
+    n, turns = c["n"], c["turns"]
+    z0, d0 = wl.gaussian_bunch(n, c["sigma_z"], c["seed"] + rank)
+    z_lo, z_hi, S = wl.slice_grid(c)
+    z, d = torch.from_numpy(z0).cuda(), torch.from_numpy(d0).cuda()
+    hist = torch.zeros(turns * (S + 2), dtype=torch.int64, device="cuda")
+    mom = torch.zeros(turns * lt.MOMENTS_DTYPE.itemsize, dtype=torch.uint8, device="cuda")
+    tr = lt.Tracker(wl.RING, "leapfrog")
+    sec = timed(lambda: tr.track_slices(z, d, n, turns, z_lo, z_hi, S, hist, None, None, sp), 2)
+    out["f4_track_slices"] = {
+        "workload": "1e7 particles x 1000 turns, one launch per turn, 64-slice histogram of z per turn",
+        "value": world * n * turns / sec, "unit": UNIT, "ms_per_turn": 1e3 * sec / turns,
+        "roofline": hbm(32, n * turns, sec)}
+    sec = timed(lambda: tr.track_slices(z, d, n, turns, z_lo, z_hi, S, hist, mom, None, sp), 2)
+    out["f4_track_slices_with_moments"] = {
+        "workload": "as f4_track_slices plus moments and membership count every turn",
+        "value": world * n * turns / sec, "unit": UNIT, "ms_per_turn": 1e3 * sec / turns,
+        "roofline": hbm(32, n * turns, sec)}
+    zs = z.clone()
+    h1 = torch.zeros(S + 2, dtype=torch.int64, device="cuda")
+    sec = timed(lambda: tr.slice_histogram(zs, n, z_lo, z_hi, S, h1, sp), 5)
+    out["f4_slice_histogram"] = {
+        "workload": "histogram of one state, 1e7 particles, 64 slices (8 B read per particle)",
+        "value": world * n / sec, "unit": "particles/s", "ms": 1e3 * sec,
+        "roofline": hbm(8, n, sec)}
+    del z, d, zs, hist, mom, tr
+
+    # f3: transverse maps, fused (4 segments x 16 + 13 longitudinal FP64 instructions) and per-turn
+    c = wl.NEXT_CONFIGS["f3_transverse"]
+    mats, twiss = wl.transverse_lattice(c["n_seg"], c["lattice_seed"])
+    tr = lt.Tracker(wl.RING, "leapfrog")
+    tr.set_transverse(mats)
+    n, turns = c["n"], c["turns"]
+    co = [torch.from_numpy(v).cuda() for v in wl.transverse_bunch(n, c["seed"] + rank, twiss)]
+    z0, d0 = wl.gaussian_bunch(n, c["sigma_z"], c["seed"] + 1 + rank)
+    z, d = torch.from_numpy(z0).cuda(), torch.from_numpy(d0).cuda()
+    sec = timed(lambda: tr.track_transverse_fused(co[0], co[1], co[2], co[3], z, d, n, turns, sp), 3)
+    instr = 16 * c["n_seg"] + FP64_INSTR_PER_PT
+    out["f3_transverse_fused"] = {
+        "workload": "1e6 particles x 1e4 turns, 4 segment matrices + the leap-frog turn, fused",
+        "value": world * n * turns / sec, "unit": UNIT, "ms": 1e3 * sec,
+        "roofline": alu(instr, n * turns, sec)}
+    sec = timed(lambda: tr.track_transverse_fused(co[0], co[1], co[2], co[3], None, None, n, turns, sp), 3)
+    out["f3_transverse_fused_4d_only"] = {
+        "workload": "as above without the longitudinal plane",
+        "value": world * n * turns / sec, "unit": UNIT, "ms": 1e3 * sec,
+        "roofline": alu(16 * c["n_seg"], n * turns, sec)}
+    del co, z, d
+    n, turns = c["per_turn_n"], c["per_turn_turns"]
+    co = [torch.from_numpy(v).cuda() for v in wl.transverse_bunch(n, c["seed"] + 2 + rank, twiss)]
+    z0, d0 = wl.gaussian_bunch(n, c["sigma_z"], c["seed"] + 3 + rank)
+    z, d = torch.from_numpy(z0).cuda(), torch.from_numpy(d0).cuda()
+    sec = timed(lambda: tr.track_transverse_per_turn(co[0], co[1], co[2], co[3], z, d, n, turns, sp), 2)
+    out["f3_transverse_per_turn"] = {
+        "workload": "1e7 particles x 200 turns, one launch per turn, six arrays through HBM (480 MB)",
+        "value": world * n * turns / sec, "unit": UNIT, "ms_per_turn": 1e3 * sec / turns,
+        "roofline": hbm(96, n * turns, sec)}
+    del co, z, d, flush
+    return out
+
 # ----------------------------------------------------------------------------- CUDA arm
 def run_cuda(args) -> None:
     import numpy as np
@@ -194,6 +309,14 @@ def run_cuda(args) -> None:
 
     peaks = measured_peaks()
     sm_max_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    if args.only_next:                                   # profiling aid: just the sec. 8(f) rows
+        nxt = bench_next(lt, wl, torch, torch.cuda.current_stream(), peaks,
+                         SMS * FP64_LANES_PER_SM * sm_max_mhz * 1e-3, max_over_ranks, world, rank)
+        if rank == 0:
+            print(json.dumps({"next": nxt}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
     cfg = wl.CONFIGS[1]
     n, turns = cfg["n"], cfg["turns"]
     z0, d0 = wl.make_bunch(cfg, seed=cfg["seed"] + rank)     # weak scaling: one bunch per rank
@@ -307,6 +430,11 @@ def run_cuda(args) -> None:
                     "clocks": clk3.summary()}
         del z3, d3
 
+    # ---- rows SURVEY.md sec. 8(f) marks "next"
+    nxt = None
+    if not args.skip_next:
+        nxt = bench_next(lt, wl, torch, stream, peaks, peak_ginstr, max_over_ranks, world, rank)
+
     # ---- FP64 probe (measured DFMA issue rate, context for the derived peak)
     probe = None
     try:
@@ -337,7 +465,7 @@ def run_cuda(args) -> None:
                        "l2": "flushed between timed iterations (256 MB fill)",
                        "parallelism": "particles sharded, no collective (weak)"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
-            "roofline": roofline, "cpu_baseline": cpu_baseline, "per_turn": per_turn,
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "per_turn": per_turn, "next": nxt,
             "wall_s_timed_region": wall,
         }))
     if world > 1:
@@ -352,6 +480,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--skip-per-turn", action="store_true")
     ap.add_argument("--skip-cpu", action="store_true")
+    ap.add_argument("--skip-next", action="store_true")
+    ap.add_argument("--only-next", action="store_true")
     args = ap.parse_args()
     import __graft_entry__ as entry
     if int(os.environ.get("LOCAL_RANK", "0")) == 0:
