@@ -206,11 +206,12 @@ static __global__ void programme_pack_kernel(const double* __restrict__ volt_sca
 // f3: transverse plane.  One turn = for every segment s in order  u <- M_s u,  u = (x, x', y, y'),
 // M_s row-major; row i is  fma(M_i3, y', fma(M_i2, y, fma(M_i1, x', M_i0 * x)))  -- the
 // association order of the definition, 16 FP64 instructions per segment and particle.
-// Up to kSegInParam matrices ride in the kernel-parameter constant bank and feed DFMA as direct
-// operands; longer lattices are read from global memory (uniform loads).
+// sm_100a has no constant-bank operands for DFMA: every matrix element has to sit in a (uniform)
+// register, and 4 matrices are 128 of them.  So the lattice is staged in shared memory and a
+// thread carries ILP particles: each element fetched (or kept in a uniform register by ptxas,
+// which hoists the loads of short lattices out of the turn loop) feeds ILP FMAs.
 // ------------------------------------------------------------------------------------------
-constexpr int kSegInParam = 4;
-struct TransConsts { double M[kSegInParam][16]; };
+constexpr int kSegUnrolled = 4;      // lattices up to this length are unrolled at compile time
 
 __device__ __forceinline__ void apply_matrix(double (&u)[4], const double* __restrict__ M) {
     double w[4];
@@ -225,42 +226,71 @@ __device__ __forceinline__ void apply_matrix(double (&u)[4], const double* __res
     for (int i = 0; i < 4; ++i) u[i] = w[i];
 }
 
-template <int NSEG>
-__device__ __forceinline__ void transverse_turn(double (&u)[4], const TransConsts& Q,
-                                                const double* __restrict__ Mg, int n_seg) {
+// 16-byte shared-memory load that ptxas may not hoist: left alone it lifts the loads of a short
+// lattice out of the turn loop into (uniform) registers and then spills the particles' state
+__device__ __forceinline__ double2 lds_pair(unsigned int addr) {
+    double2 r;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "r"(addr));
+    return r;
+}
+
+// the same for ILP particles of one thread: a matrix row is read once (two 16-byte loads from
+// shared memory at byte address M) and feeds 4*ILP FP64 instructions
+template <int ILP>
+__device__ __forceinline__ void apply_matrix_ilp(double (&u)[ILP][4], unsigned int M) {
+    double w[ILP][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const double2 a = lds_pair(M + 32u * i), b = lds_pair(M + 32u * i + 16u);
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            double acc = __dmul_rn(a.x, u[j][0]);
+            acc = __fma_rn(a.y, u[j][1], acc);
+            acc = __fma_rn(b.x, u[j][2], acc);
+            w[j][i] = __fma_rn(b.y, u[j][3], acc);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < ILP; ++j)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) u[j][i] = w[j][i];
+}
+
+template <int NSEG, int ILP>
+__device__ __forceinline__ void transverse_turn(double (&u)[ILP][4], unsigned int lat, int n_seg) {
     if (NSEG > 0) {
 #pragma unroll
-        for (int s = 0; s < NSEG; ++s) apply_matrix(u, Q.M[s]);
+        for (int s = 0; s < NSEG; ++s) apply_matrix_ilp<ILP>(u, lat + 128u * s);
     } else {
-        for (int s = 0; s < n_seg; ++s) {
-            double M[16];
-#pragma unroll
-            for (int k = 0; k < 8; ++k) {
-                const double2 e = __ldg(reinterpret_cast<const double2*>(Mg + 16 * (size_t)s) + k);
-                M[2 * k] = e.x; M[2 * k + 1] = e.y;
-            }
-            apply_matrix(u, M);
-        }
+#pragma unroll 1
+        for (int s = 0; s < n_seg; ++s) apply_matrix_ilp<ILP>(u, lat + 128u * s);
     }
 }
 
 // Fused multi-turn transverse kernel: the persistent, ticketed work queue of
-// fused_persistent_kernel (items = chunk of item_turns turns x group of 32 particles) with the
+// fused_persistent_kernel (items = chunk of item_turns turns x group of 32*ILP particles) with the
 // four transverse coordinates -- and, when LONGI, the leap-frog single-harmonic longitudinal
 // turn of the same particle (fast path: phase state, merged drifts) -- held in registers.
-template <int NSEG, bool LONGI>
-__global__ void __launch_bounds__(1024, 1)
+// Particle j of a lane is element  g*32*ILP + j*32 + lane  (coalesced).  The arithmetic per
+// particle does not depend on ILP, so every launch shape returns the same bits.
+template <int NSEG, bool LONGI, int ILP>
+__global__ void __launch_bounds__(ILP == 1 ? 1024 : 512, 1)
 transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp_arr,
                              double* __restrict__ y_arr, double* __restrict__ yp_arr,
                              double* __restrict__ z_arr, double* __restrict__ d_arr, size_t n,
                              unsigned int turns, unsigned int item_turns, int first_launch,
                              int last_launch, int dynamic, unsigned long long* __restrict__ ticket,
                              unsigned int* __restrict__ done, const double* __restrict__ Mg,
-                             int n_seg, const __grid_constant__ TransConsts Q,
-                             const __grid_constant__ MapConsts<double> P) {
-    extern __shared__ unsigned char residency_cap[];   // unused: sized to cap CTAs per SM
+                             int n_seg, const __grid_constant__ MapConsts<double> P) {
+    // dynamic shared memory: the lattice; the request is padded to cap the CTAs per SM
+    extern __shared__ double2 lattice2[];
+    for (int k = threadIdx.x; k < 8 * n_seg; k += blockDim.x)
+        lattice2[k] = __ldg(reinterpret_cast<const double2*>(Mg) + k);
+    __syncthreads();
+    const unsigned int lat = (unsigned int)__cvta_generic_to_shared(lattice2);
+    constexpr unsigned int G = 32u * ILP;
     const unsigned int lane = threadIdx.x & 31u;
-    const unsigned long long groups = (n + 31) / 32;
+    const unsigned long long groups = (n + G - 1) / G;
     const unsigned int nchunks = (turns + item_turns - 1) / item_turns;
     const unsigned long long total = groups * nchunks;
     const unsigned long long slots = (unsigned long long)gridDim.x * (blockDim.x >> 5);
@@ -279,35 +309,48 @@ transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp
         if (c > 0) {
             while (ld_acquire_u32(done + g) < c) __nanosleep(64);
         }
-        const size_t i = (size_t)g * 32 + lane;
-        const bool live = i < n;
-        double u[4], v = 0.0, dl = 0.0;
-        u[0] = live ? __ldcg(x_arr + i) : 0.0;
-        u[1] = live ? __ldcg(xp_arr + i) : 0.0;
-        u[2] = live ? __ldcg(y_arr + i) : 0.0;
-        u[3] = live ? __ldcg(yp_arr + i) : 0.0;
+        const size_t i0 = (size_t)g * G + lane;
         const int first = first_launch && c == 0;
         const int last = last_launch && c == nchunks - 1;
         const unsigned int nt = (c == nchunks - 1) ? turns - c * item_turns : item_turns;
-        if (LONGI) {
-            v = live ? __ldcg(z_arr + i) : 0.0;
-            dl = live ? __ldcg(d_arr + i) : 0.0;
-            if (first) v = __fma_rn(-P.drift_lead, dl, __dmul_rn(v, P.to_phase));
+        double u[ILP][4], v[ILP], dl[ILP];
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            const size_t i = i0 + 32u * j;
+            const bool live = i < n;
+            u[j][0] = live ? __ldcg(x_arr + i) : 0.0;
+            u[j][1] = live ? __ldcg(xp_arr + i) : 0.0;
+            u[j][2] = live ? __ldcg(y_arr + i) : 0.0;
+            u[j][3] = live ? __ldcg(yp_arr + i) : 0.0;
+            v[j] = 0.0; dl[j] = 0.0;
+            if (LONGI) {
+                v[j] = live ? __ldcg(z_arr + i) : 0.0;
+                dl[j] = live ? __ldcg(d_arr + i) : 0.0;
+                if (first) v[j] = __fma_rn(-P.drift_lead, dl[j], __dmul_rn(v[j], P.to_phase));
+            }
         }
-#pragma unroll 2
+#pragma unroll 1
         for (unsigned int k = 1; k < nt; ++k) {
-            transverse_turn<NSEG>(u, Q, Mg, n_seg);
-            if (LONGI) turn_fast<double, kLeapfrog, 1, true>(v, dl, P, P.drift_merged);
+            transverse_turn<NSEG, ILP>(u, lat, n_seg);
+            if (LONGI) {
+#pragma unroll
+                for (int j = 0; j < ILP; ++j)
+                    turn_fast<double, kLeapfrog, 1, true>(v[j], dl[j], P, P.drift_merged);
+            }
         }
-        transverse_turn<NSEG>(u, Q, Mg, n_seg);
-        if (LONGI) {
-            turn_fast<double, kLeapfrog, 1, true>(v, dl, P, last ? P.drift_trail : P.drift_merged);
-            if (last) v = __dmul_rn(v, P.from_phase);
-        }
-        if (live) {
-            __stcg(x_arr + i, u[0]); __stcg(xp_arr + i, u[1]);
-            __stcg(y_arr + i, u[2]); __stcg(yp_arr + i, u[3]);
-            if (LONGI) { __stcg(z_arr + i, v); __stcg(d_arr + i, dl); }
+        transverse_turn<NSEG, ILP>(u, lat, n_seg);
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            const size_t i = i0 + 32u * j;
+            if (LONGI) {
+                turn_fast<double, kLeapfrog, 1, true>(v[j], dl[j], P, last ? P.drift_trail : P.drift_merged);
+                if (last) v[j] = __dmul_rn(v[j], P.from_phase);
+            }
+            if (i < n) {
+                __stcg(x_arr + i, u[j][0]); __stcg(xp_arr + i, u[j][1]);
+                __stcg(y_arr + i, u[j][2]); __stcg(yp_arr + i, u[j][3]);
+                if (LONGI) { __stcg(z_arr + i, v[j]); __stcg(d_arr + i, dl[j]); }
+            }
         }
         if (nchunks > 1) {
             __threadfence();

@@ -279,28 +279,58 @@ int ensure_lattice(lt_tracker* tr, cudaStream_t st) {
     return LT_OK;
 }
 
-template <int NSEG, bool LONGI>
+// launch shape of the fused transverse kernel: ILP particles per thread (4 or 2 at 4 warps per
+// sub-partition, 128 registers per thread; 1 at the plan of the longitudinal kernel), the largest
+// ILP that still fills one wave of warps; dynamic chunk scheduling beyond one wave
+struct TransPlan { int ilp; PersistentPlan pl; };
+
+TransPlan plan_transverse(const lt_tracker* tr, size_t n, unsigned long long turns) {
+    TransPlan tp;
+    tp.ilp = 1;
+    const unsigned long long slots = (unsigned long long)tr->sm_count * 16;
+    int ilp = 0;
+    if (tr->fused_ilp == 1 || tr->fused_ilp == 2 || tr->fused_ilp == 4) ilp = (int)tr->fused_ilp;
+    else if ((n + 127) / 128 >= slots) ilp = 4;
+    else if ((n + 63) / 64 >= slots) ilp = 2;
+    else ilp = 1;
+    if (ilp == 1) {
+        tp.pl = plan_persistent(tr, n, turns);
+        return tp;
+    }
+    tp.ilp = ilp;
+    const unsigned long long groups = (n + 32 * ilp - 1) / (32 * ilp);
+    PersistentPlan pl = {0, 4, 1, 512, 0, true};
+    pl.dynamic = (groups > slots || tr->fused_mode == 3) && tr->fused_mode != 2;
+    if (pl.dynamic) {
+        unsigned long long it = tr->item_turns > 0
+                                    ? (unsigned long long)tr->item_turns
+                                    : std::min<unsigned long long>(1024, std::max<unsigned long long>(256, turns / 64));
+        pl.item_turns = (unsigned int)std::min<unsigned long long>(it, turns);
+    }
+    tp.pl = pl;
+    return tp;
+}
+
+template <int NSEG, bool LONGI, int ILP>
 cudaError_t launch_transverse_one(double* x, double* xp, double* y, double* yp, double* z, double* d,
                                   size_t n, unsigned int turns, unsigned int item_turns, int first, int last,
-                                  const PersistentPlan& pl, const lt_tracker* tr, const TransConsts& Q,
-                                  cudaStream_t st) {
-    auto kern = transverse_persistent_kernel<NSEG, LONGI>;
-    const int smem = residency_smem(pl);
+                                  const PersistentPlan& pl, const lt_tracker* tr, cudaStream_t st) {
+    auto kern = transverse_persistent_kernel<NSEG, LONGI, ILP>;
+    const int smem = residency_smem(pl);                 // >= the lattice (256 x 128 B)
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     kern<<<tr->sm_count * pl.ctas_per_sm, pl.threads, smem, st>>>(
         x, xp, y, yp, z, d, n, turns, item_turns, first, last, pl.dynamic, tr->sched,
-        reinterpret_cast<unsigned int*>(tr->sched + 1), tr->lattice_dev, tr->n_seg, Q, tr->c64);
+        reinterpret_cast<unsigned int*>(tr->sched + 1), tr->lattice_dev, tr->n_seg, tr->c64);
     return cudaGetLastError();
 }
 
-template <bool LONGI>
-cudaError_t launch_transverse(double* x, double* xp, double* y, double* yp, double* z, double* d,
-                              size_t n, unsigned int turns, unsigned int item_turns, int first, int last,
-                              const PersistentPlan& pl, const lt_tracker* tr, const TransConsts& Q,
-                              cudaStream_t st) {
-#define LT_TV(NS) launch_transverse_one<NS, LONGI>(x, xp, y, yp, z, d, n, turns, item_turns, first, last, pl, tr, Q, st)
-    switch (tr->n_seg <= kSegInParam ? tr->n_seg : 0) {
+template <bool LONGI, int ILP>
+cudaError_t launch_transverse_ilp(double* x, double* xp, double* y, double* yp, double* z, double* d,
+                                  size_t n, unsigned int turns, unsigned int item_turns, int first, int last,
+                                  const PersistentPlan& pl, const lt_tracker* tr, cudaStream_t st) {
+#define LT_TV(NS) launch_transverse_one<NS, LONGI, ILP>(x, xp, y, yp, z, d, n, turns, item_turns, first, last, pl, tr, st)
+    switch (tr->n_seg <= kSegUnrolled ? tr->n_seg : 0) {
         case 1: return LT_TV(1);
         case 2: return LT_TV(2);
         case 3: return LT_TV(3);
@@ -308,6 +338,15 @@ cudaError_t launch_transverse(double* x, double* xp, double* y, double* yp, doub
         default: return LT_TV(0);
     }
 #undef LT_TV
+}
+
+template <bool LONGI>
+cudaError_t launch_transverse(double* x, double* xp, double* y, double* yp, double* z, double* d,
+                              size_t n, unsigned int turns, unsigned int item_turns, int first, int last,
+                              const TransPlan& tp, const lt_tracker* tr, cudaStream_t st) {
+    if (tp.ilp == 4) return launch_transverse_ilp<LONGI, 4>(x, xp, y, yp, z, d, n, turns, item_turns, first, last, tp.pl, tr, st);
+    if (tp.ilp == 2) return launch_transverse_ilp<LONGI, 2>(x, xp, y, yp, z, d, n, turns, item_turns, first, last, tp.pl, tr, st);
+    return launch_transverse_ilp<LONGI, 1>(x, xp, y, yp, z, d, n, turns, item_turns, first, last, tp.pl, tr, st);
 }
 
 int check_transverse_args(lt_tracker* tr, double* x, double* xp, double* y, double* yp, double* z,
@@ -341,19 +380,17 @@ int track_transverse_fused(lt_tracker* tr, double* x, double* xp, double* y, dou
     if (rc) return rc;
     rc = ensure_sched(tr, n);
     if (rc) return rc;
-    TransConsts Q;
-    std::memset(&Q, 0, sizeof(Q));
-    std::memcpy(Q.M, tr->lattice_host, (size_t)std::min(tr->n_seg, kSegInParam) * 16 * sizeof(double));
     const bool longi = z && longitudinal_rides_along(tr, true);
-    const PersistentPlan pl = plan_persistent(tr, n, turns);
+    const TransPlan tp = plan_transverse(tr, n, turns);
+    const PersistentPlan& pl = tp.pl;
     unsigned long long done = 0;
     while (done < turns) {
         const unsigned long long chunk = std::min<unsigned long long>(turns - done, (unsigned long long)tr->chunk_turns);
         const int first = done == 0, last = done + chunk == turns;
         const unsigned int item = pl.dynamic ? std::min<unsigned int>(pl.item_turns, (unsigned int)chunk) : (unsigned int)chunk;
         if (pl.dynamic) LT_CUDA(tr, cudaMemsetAsync(tr->sched, 0, 8 + 4 * ((n + 31) / 32), st));
-        cudaError_t e = longi ? launch_transverse<true>(x, xp, y, yp, z, d, n, (unsigned)chunk, item, first, last, pl, tr, Q, st)
-                              : launch_transverse<false>(x, xp, y, yp, z, d, n, (unsigned)chunk, item, first, last, pl, tr, Q, st);
+        cudaError_t e = longi ? launch_transverse<true>(x, xp, y, yp, z, d, n, (unsigned)chunk, item, first, last, tp, tr, st)
+                              : launch_transverse<false>(x, xp, y, yp, z, d, n, (unsigned)chunk, item, first, last, tp, tr, st);
         LT_CUDA(tr, e);
         tr->launches++;
         done += chunk;
@@ -364,7 +401,7 @@ int track_transverse_fused(lt_tracker* tr, double* x, double* xp, double* y, dou
     }
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
-    tr->last_ilp = 1;
+    tr->last_ilp = tp.ilp;
     tr->last_mode = pl.dynamic ? 3 : 2;
     tr->last_item_turns = pl.dynamic ? pl.item_turns : 0;
     return LT_OK;
