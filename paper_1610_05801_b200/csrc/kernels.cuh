@@ -222,14 +222,61 @@ __device__ __forceinline__ void turn_fast(T& v, T& delta, const MapConsts<T>& P,
 template <typename T, int INTEG, int HARM, bool SPLIT, int ILP, bool FQ, bool PROG = false>
 __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int turns, int first,
                                         int last, const MapConsts<T>& P,
-                                        const double2* __restrict__ prog = nullptr) {
+                                        const double2* __restrict__ prog = nullptr,
+                                        double2* __restrict__ stage = nullptr) {
     typedef Real<T> R;
+    if (PROG) {
+        // RF programme.  The table is read 32 turns ahead: lane l fetches entry t0 + 32 + l
+        // while the warp works through entries t0 .. t0 + 31 out of its private 512-byte
+        // buffer in shared memory (one broadcast LDS.128 per turn).  A per-turn uniform LDG
+        // left the warps waiting on L2 once per 128-byte line (long-scoreboard stalls, 76 %
+        // of the FP64 peak; profiles/r1_next_rows_ncu.md).
+        const unsigned int lane = threadIdx.x & 31u;
+        if (!SPLIT && first) {
+#pragma unroll
+            for (int j = 0; j < ILP; ++j) {
+                x[j] = R::mul(x[j], P.to_phase);
+                if (INTEG != kEulerCromer) x[j] = R::fma(-P.drift_lead, dl[j], x[j]);
+            }
+        }
+        // the fast path peels the last turn (its trailing drift differs at the end of a call)
+        const unsigned int nmain = SPLIT ? turns : turns - 1;
+        double2 tail = make_double2(1.0, 0.0);
+        if (!SPLIT) tail = __ldg(prog + (turns - 1));
+        double2 nxt = make_double2(1.0, 0.0);
+        if (lane < nmain) nxt = __ldg(prog + lane);
+        for (unsigned int t0 = 0; t0 < nmain; t0 += 32) {
+            __syncwarp();
+            stage[lane] = nxt;
+            __syncwarp();
+            if (t0 + 32 + lane < nmain) nxt = __ldg(prog + t0 + 32 + lane);
+            const unsigned int m = min(32u, nmain - t0);
+            constexpr int kUnrollP = (INTEG == kRuth4 || HARM != 1) ? 4 : 16;
+#pragma unroll kUnrollP
+            for (unsigned int k = 0; k < m; ++k) {
+                const double2 e = stage[k];
+                const T a = (T)e.x, p = (T)e.y;
+#pragma unroll
+                for (int j = 0; j < ILP; ++j) {
+                    if (SPLIT) turn_exact<T, INTEG, HARM, true>(x[j], dl[j], P, a, p);
+                    else turn_fast<T, INTEG, HARM, FQ, true>(x[j], dl[j], P, P.drift_merged, a, p);
+                }
+            }
+        }
+        if (!SPLIT) {
+            const T trailing = last ? P.drift_trail : P.drift_merged;
+#pragma unroll
+            for (int j = 0; j < ILP; ++j) {
+                turn_fast<T, INTEG, HARM, FQ, true>(x[j], dl[j], P, trailing, (T)tail.x, (T)tail.y);
+                if (last) x[j] = R::mul(x[j], P.from_phase);
+            }
+        }
+        return;
+    }
     if (SPLIT) {
         for (unsigned int t = 0; t < turns; ++t) {
-            T a = T(1), p = T(0);
-            if (PROG) { const double2 e = __ldg(prog + t); a = (T)e.x; p = (T)e.y; }
 #pragma unroll
-            for (int j = 0; j < ILP; ++j) turn_exact<T, INTEG, HARM, PROG>(x[j], dl[j], P, a, p);
+            for (int j = 0; j < ILP; ++j) turn_exact<T, INTEG, HARM, false>(x[j], dl[j], P);
         }
     } else {
         if (first) {
@@ -244,18 +291,14 @@ __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int 
         constexpr int kUnroll = (INTEG == kRuth4 || HARM != 1 || ILP > 2) ? 4 : LT_TURN_UNROLL / ILP;
 #pragma unroll kUnroll
         for (unsigned int t = 1; t < turns; ++t) {
-            T a = T(1), p = T(0);
-            if (PROG) { const double2 e = __ldg(prog + (t - 1)); a = (T)e.x; p = (T)e.y; }
 #pragma unroll
             for (int j = 0; j < ILP; ++j)
-                turn_fast<T, INTEG, HARM, FQ, PROG>(x[j], dl[j], P, P.drift_merged, a, p);
+                turn_fast<T, INTEG, HARM, FQ, false>(x[j], dl[j], P, P.drift_merged);
         }
         const T trailing = last ? P.drift_trail : P.drift_merged;
-        T a = T(1), p = T(0);
-        if (PROG) { const double2 e = __ldg(prog + (turns - 1)); a = (T)e.x; p = (T)e.y; }
 #pragma unroll
         for (int j = 0; j < ILP; ++j) {
-            turn_fast<T, INTEG, HARM, FQ, PROG>(x[j], dl[j], P, trailing, a, p);
+            turn_fast<T, INTEG, HARM, FQ, false>(x[j], dl[j], P, trailing);
             if (last) x[j] = R::mul(x[j], P.from_phase);
         }
     }
@@ -359,7 +402,7 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
                         unsigned long long* __restrict__ ticket, unsigned int* __restrict__ done,
                         const __grid_constant__ MapConsts<T> P,
                         const double2* __restrict__ prog = nullptr) {
-    extern __shared__ unsigned char residency_cap[];   // unused: sized to cap CTAs per SM
+    extern __shared__ __align__(16) unsigned char residency_cap[];   // sized to cap CTAs per SM; PROG: 512 B per warp of staged programme entries
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned long long groups = (n + 31) / 32;
     const unsigned int nchunks = (turns + item_turns - 1) / item_turns;
@@ -389,8 +432,9 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
         const int first = first_launch && c == 0;
         const int last = last_launch && c == nchunks - 1;
         const unsigned int nt = (c == nchunks - 1) ? turns - c * item_turns : item_turns;
-        advance<T, INTEG, HARM, SPLIT, 1, FQ, PROG>(x, dl, nt, first, last, P,
-                                                    PROG ? prog + (size_t)c * item_turns : nullptr);
+        advance<T, INTEG, HARM, SPLIT, 1, FQ, PROG>(
+            x, dl, nt, first, last, P, PROG ? prog + (size_t)c * item_turns : nullptr,
+            PROG ? reinterpret_cast<double2*>(residency_cap) + (threadIdx.x & ~31u) : nullptr);
         if (i < n) { __stcg(z_arr + i, x[0]); __stcg(d_arr + i, dl[0]); }
         if (nchunks > 1) {
             __threadfence();
