@@ -182,15 +182,34 @@ static __global__ void advance_cursor_kernel(unsigned long long* cursor, unsigne
     *cursor += by;
 }
 
-// Histogram of a given state (lt_slice_histogram): grid-stride read of z only (8 B per particle).
+// Histogram of a given state (lt_slice_histogram): 8 B read per particle.  Persistent CTAs walk
+// tiles of blockDim.x * 2 * UNR particles; the UNR 16-byte loads of a tile are all issued before
+// the first shared-memory atomic, so that every thread keeps 64 B in flight (one 8-byte load per
+// grid-stride step left the kernel latency-bound at 35 % of the copy rate).  A z array that is
+// only 8-byte aligned is shifted by one element (`head`), which the first thread takes alone.
+template <int UNR>
 static __global__ void slice_histogram_kernel(const double* __restrict__ z_arr, size_t n,
                                        const __grid_constant__ TurnExtras X) {
     extern __shared__ unsigned int slice_smem[];
     SliceAcc sl;
     sl.init(X, 0ULL, slice_smem);
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
-         i += (size_t)gridDim.x * blockDim.x)
-        sl.add(z_arr[i]);
+    const size_t head = ((reinterpret_cast<uintptr_t>(z_arr) & 15u) != 0 && n > 0) ? 1 : 0;
+    if (head && blockIdx.x == 0 && threadIdx.x == 0) sl.add(z_arr[0]);
+    const double* __restrict__ zb = z_arr + head;
+    const size_t m = n - head;
+    const size_t tile = (size_t)blockDim.x * 2 * UNR;
+    for (size_t base = (size_t)blockIdx.x * tile; base < m; base += (size_t)gridDim.x * tile) {
+        double2 v[UNR];
+        if (base + tile <= m) {
+#pragma unroll
+            for (int u = 0; u < UNR; ++u)
+                v[u] = __ldcs(reinterpret_cast<const double2*>(zb + base) + u * blockDim.x + threadIdx.x);
+#pragma unroll
+            for (int u = 0; u < UNR; ++u) { sl.add(v[u].x); sl.add(v[u].y); }
+        } else {
+            for (size_t i = base + threadIdx.x; i < m; i += blockDim.x) sl.add(zb[i]);
+        }
+    }
     sl.flush();
 }
 

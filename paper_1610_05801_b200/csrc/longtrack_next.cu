@@ -504,10 +504,11 @@ int lt_slice_histogram(lt_tracker* tr, const double* z_dev, size_t n, double z_l
     if (n == 0) return LT_OK;
     const ExtraArgs a = {nullptr, nullptr, hist_dev, z_lo, z_hi, n_slices};
     const TurnExtras X = make_extras(tr, a, 0);
-    size_t g = (n + 255) / 256;
+    constexpr int kUnr = 4;                                   // 64 B in flight per thread
+    size_t g = (n + 256 * 2 * kUnr - 1) / (256 * 2 * kUnr);
     g = std::max<size_t>(1, std::min<size_t>(g, (size_t)tr->sm_count * 8));
     const size_t smem = (size_t)X.replicas * ((size_t)n_slices + 2) * sizeof(unsigned int);
-    slice_histogram_kernel<<<(unsigned)g, 256, smem, st>>>(z_dev, n, X);
+    slice_histogram_kernel<kUnr><<<(unsigned)g, 256, smem, st>>>(z_dev, n, X);
     LT_CUDA(tr, cudaGetLastError());
     tr->launches++;
     return LT_OK;

@@ -198,6 +198,23 @@ def test_slice_histogram_of_a_state_is_exact(S):
     assert np.array_equal(gpu_hist(tr, z, -0.7, 0.7, S), oracle.slice_histogram(z, -0.7, 0.7, S))
 
 
+@pytest.mark.parametrize("n", [1, 2, 2047, 2048, 2049, 4097, 1_000_001])
+@pytest.mark.parametrize("offset", [0, 1])
+def test_slice_histogram_sizes_around_a_tile_and_8_byte_alignment(n, offset):
+    """The kernel walks tiles of 2048 particles with 16-byte loads: sizes around the tile, a
+    ragged tail, and a z pointer that is only 8-byte aligned (view starting at element 1)."""
+    rng = np.random.default_rng(77 + n)
+    z = rng.normal(0.0, 0.3, n + offset)
+    tr, _ = both()
+    zt = dev(z)[offset:]
+    assert zt.data_ptr() % 16 == 8 * offset
+    h = torch.full((64 + 2,), -1, dtype=torch.int64, device="cuda")
+    tr.slice_histogram(zt, n, -0.7, 0.7, 64, h, stream_ptr())
+    torch.cuda.synchronize()
+    assert np.array_equal(h.cpu().numpy().astype(np.uint64),
+                          oracle.slice_histogram(z[offset:], -0.7, 0.7, 64))
+
+
 def test_slice_edges_on_a_dyadic_grid_and_empty_input():
     tr, _ = both()
     S = 8
