@@ -103,6 +103,14 @@ def lib():
         L.lto_track_programme_ld.restype = None
         L.lto_track_programme_moments.argtypes = [pp, dp, dp, c_size_t, c_ulonglong, dp, dp, c_void_p]
         L.lto_track_programme_moments.restype = None
+        L.lto_track_ramp.argtypes = [pp, dp, dp, c_size_t, c_ulonglong, dp, dp, dp]
+        L.lto_track_ramp.restype = None
+        L.lto_track_ramp_ld.argtypes = [pp, c_void_p, c_void_p, c_size_t, c_ulonglong, dp, dp, dp]
+        L.lto_track_ramp_ld.restype = None
+        L.lto_track_ramp_moments.argtypes = [pp, dp, dp, c_size_t, c_ulonglong, dp, dp, dp, c_void_p]
+        L.lto_track_ramp_moments.restype = None
+        L.lto_ramp_numbers.argtypes = [pp, c_double, dp, dp, dp, dp, dp]
+        L.lto_ramp_numbers.restype = None
         L.lto_slice_histogram.argtypes = [dp, c_size_t, c_double, c_double, c_int, ull]
         L.lto_slice_histogram.restype = None
         L.lto_track_slices.argtypes = [pp, dp, dp, c_size_t, c_ulonglong, c_double, c_double,
@@ -261,6 +269,58 @@ def track_programme_moments(p: Params, z, delta, volt_scale, phase_off):
     lib().lto_track_programme_moments(ctypes.byref(p), zp, dp_, z.size, a.size, ap, sp,
                                       out.ctypes.data)
     return z, d, out
+
+
+def _ramp_tables(p0c, volt_scale, phase_off):
+    pc, pcp = _f64(p0c)
+    turns = pc.size - 1
+    assert turns >= 0
+    keep = [pc]
+    ap = sp = None
+    if volt_scale is not None:
+        a, ap = _f64(volt_scale)
+        assert a.size == turns
+        keep.append(a)
+    if phase_off is not None:
+        s, sp = _f64(phase_off)
+        assert s.size == turns
+        keep.append(s)
+    return turns, pcp, ap, sp, keep
+
+
+def track_ramp(p: Params, z, delta, p0c, volt_scale=None, phase_off=None):
+    """f2 with an energy ramp (G32): p0c has turns+1 entries; returns new (z, delta)."""
+    z, zp = _copy(z)
+    d, dp_ = _copy(delta)
+    turns, pcp, ap, sp, _keep = _ramp_tables(p0c, volt_scale, phase_off)
+    lib().lto_track_ramp(ctypes.byref(p), zp, dp_, z.size, turns, pcp, ap, sp)
+    return z, d
+
+
+def track_ramp_ld(p: Params, z, delta, p0c, volt_scale=None, phase_off=None):
+    z = np.ascontiguousarray(np.array(z, dtype=np.longdouble, copy=True).ravel())
+    d = np.ascontiguousarray(np.array(delta, dtype=np.longdouble, copy=True).ravel())
+    assert z.dtype.itemsize == 16
+    turns, pcp, ap, sp, _keep = _ramp_tables(p0c, volt_scale, phase_off)
+    lib().lto_track_ramp_ld(ctypes.byref(p), z.ctypes.data, d.ctypes.data, z.size, turns, pcp, ap, sp)
+    return z, d
+
+
+def track_ramp_moments(p: Params, z, delta, p0c, volt_scale=None, phase_off=None):
+    z, zp = _copy(z)
+    d, dp_ = _copy(delta)
+    turns, pcp, ap, sp, _keep = _ramp_tables(p0c, volt_scale, phase_off)
+    out = np.zeros(turns, dtype=MOMENTS_DTYPE)
+    lib().lto_track_ramp_moments(ctypes.byref(p), zp, dp_, z.size, turns, pcp, ap, sp,
+                                 out.ctypes.data)
+    return z, d, out
+
+
+def ramp_numbers(p: Params, p0c: float) -> dict:
+    """mc2, beta, eta, A, d at reference momentum p0c (G32)."""
+    v = [ctypes.c_double() for _ in range(5)]
+    lib().lto_ramp_numbers(ctypes.byref(p), float(p0c), *[ctypes.byref(x) for x in v])
+    return dict(zip(("mc2", "beta", "eta", "A", "d"), (x.value for x in v)))
 
 
 def slice_histogram(z, z_lo: float, z_hi: float, n_slices: int):

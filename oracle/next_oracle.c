@@ -19,6 +19,7 @@
 #define NAME(x) n64_##x
 #include "map.inc"
 #include "programme.inc"
+#include "ramp.inc"
 #undef REAL
 #undef SIN
 #undef SQRT
@@ -34,6 +35,7 @@
 #define NAME(x) n80_##x
 #include "map.inc"
 #include "programme.inc"
+#include "ramp.inc"
 #undef REAL
 #undef SIN
 #undef SQRT
@@ -74,6 +76,45 @@ void lto_track_programme_moments(const lto_params *p, double *z, double *delta, 
         n64_prog_track_particles(p, z, delta, n, 1ULL, volt_scale + t, phase_off + t);
         lto_moments_of(p, z, delta, n, &out[t]);
     }
+}
+
+/* ---- f2, energy ramp (reading G32) ------------------------------------------------------- */
+void lto_track_ramp(const lto_params *p, double *z, double *delta, size_t n,
+                    unsigned long long turns, const double *p0c, const double *volt_scale,
+                    const double *phase_off)
+{
+    n64_ramp_track_particles(p, z, delta, n, turns, p0c, volt_scale, phase_off);
+}
+
+void lto_track_ramp_ld(const lto_params *p, long double *z, long double *delta, size_t n,
+                       unsigned long long turns, const double *p0c, const double *volt_scale,
+                       const double *phase_off)
+{
+    n80_ramp_track_particles(p, z, delta, n, turns, p0c, volt_scale, phase_off);
+}
+
+void lto_track_ramp_moments(const lto_params *p, double *z, double *delta, size_t n,
+                            unsigned long long turns, const double *p0c, const double *volt_scale,
+                            const double *phase_off, lto_moments *out)
+{
+    unsigned long long t;
+    for (t = 0; t < turns; ++t) {
+        n64_ramp_track_particles(p, z, delta, n, 1ULL, p0c + t, volt_scale ? volt_scale + t : NULL,
+                                 phase_off ? phase_off + t : NULL);
+        lto_moments_of(p, z, delta, n, &out[t]);
+    }
+}
+
+void lto_ramp_numbers(const lto_params *p, double p0c, double *mc2, double *beta, double *eta,
+                      double *A, double *d)
+{
+    const double m = n64_ramp_rest_energy(p);
+    const n64_ramp_point q = n64_ramp_at(p, m, p0c);
+    if (mc2) *mc2 = m;
+    if (beta) *beta = (double)p->charge_e * p->voltage_V / (q.A * p0c);
+    if (eta) *eta = 2.0 * q.d / p->circumference_m;
+    if (A) *A = q.A;
+    if (d) *d = q.d;
 }
 
 /* ---- f4 ---------------------------------------------------------------------------------- */

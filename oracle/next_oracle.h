@@ -40,6 +40,28 @@ void lto_track_programme_moments(const lto_params *p, double *z, double *delta, 
                                  unsigned long long turns, const double *volt_scale,
                                  const double *phase_off, lto_moments *out);
 
+/* ---- f2, energy ramp (reading G32; the formulas are restated in ramp.inc) ----------------
+ * p0c[0 .. turns]: reference momentum x c (eV) before turn 1 and after every turn.
+ * volt_scale / phase_off: as above, or NULL for a_t = 1 / psi_t = 0.  p->phi_s must be 0.
+ *   sub-step(tau, pb -> pa):  z -= tau d(pb) delta
+ *                             delta = (delta + tau a_t A(pb) [sin(kappa z + psi_t) + r sin(2(kappa z + psi_t))]
+ *                                      - (pa - pb)/pb) * (pb/pa)
+ *                             z -= tau d(pa) delta
+ * with A(p) = qV/(beta(p) p), d(p) = eta(p) C/2, beta, eta from p and mc2 = p0c_create/(beta gamma). */
+void lto_track_ramp(const lto_params *p, double *z, double *delta, size_t n,
+                    unsigned long long turns, const double *p0c, const double *volt_scale,
+                    const double *phase_off);
+void lto_track_ramp_ld(const lto_params *p, long double *z, long double *delta, size_t n,
+                       unsigned long long turns, const double *p0c, const double *volt_scale,
+                       const double *phase_off);
+/* out[t] = moments of the state after turn t+1 (membership: the stationary bucket of p) */
+void lto_track_ramp_moments(const lto_params *p, double *z, double *delta, size_t n,
+                            unsigned long long turns, const double *p0c, const double *volt_scale,
+                            const double *phase_off, lto_moments *out);
+/* the momentum-dependent ring numbers at reference momentum p0c (for the tests and recipes) */
+void lto_ramp_numbers(const lto_params *p, double p0c, double *mc2, double *beta, double *eta,
+                      double *A, double *d);
+
 /* ---- f4: longitudinal slicing (reading G29) --------------------------------------------
  * Uniform slices of z over [z_lo, z_hi): inv = S / (z_hi - z_lo);
  *   z < z_lo            -> hist[0]     ("below")

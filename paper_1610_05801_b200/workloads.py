@@ -155,6 +155,40 @@ NEXT_CONFIGS = dict(
 )
 
 
+def ramp_ring_numbers(p0c, ring: dict = RING):
+    """A(p) = qV/(beta(p) p) and eta(p) at reference momentum p0c (array or scalar), with the rest
+    energy mc2 = p0c_create/(beta gamma) (G32).  Part of the *input recipe* only: it
+    places the RF phase programme on the synchronous phase."""
+    g = ring["gamma"]
+    mc2 = ring["p0c_eV"] / (math.sqrt(1.0 - 1.0 / g ** 2) * g)
+    bg = np.asarray(p0c, dtype=np.float64) / mc2
+    g2 = 1.0 + bg * bg
+    beta = bg / np.sqrt(g2)
+    return dict(mc2=mc2, beta=beta, eta=ring["alpha_c"] - 1.0 / g2,
+                A=ring.get("charge_e", 1.0) * ring["voltage_V"] / (beta * np.asarray(p0c, dtype=np.float64)))
+
+
+def energy_ramp(turns: int, p_start: float, p_end: float, ring: dict = RING,
+                volt_scale: float = 1.0):
+    """f2 with acceleration: (p0c[turns+1], volt_scale[turns], phase_off[turns]).
+
+    The reference momentum goes from p_start to p_end with a rate that starts and ends at zero,
+    p(t) = p_start + (p_end - p_start) (t/N - sin(2 pi t/N)/(2 pi)) (a synchrotron's ramp is
+    rounded at both ends so that the bunch is not kicked into a dipole oscillation); constant
+    voltage; the RF phase programme keeps the reference particle synchronous,
+    psi_t = arcsin(D_t / (p0c[t] a_t A(p0c[t]))) (G32).  The paper gives no ramp."""
+    t = np.arange(turns + 1, dtype=np.float64)
+    N = float(max(turns, 1))
+    p0c = p_start + (p_end - p_start) * (t / N - np.sin(2.0 * np.pi * t / N) / (2.0 * np.pi))
+    p0c[0], p0c[-1] = p_start, p_end
+    a = np.full(turns, float(volt_scale))
+    A = ramp_ring_numbers(p0c[:-1], ring)["A"]
+    s = np.diff(p0c) / (p0c[:-1] * a * A)
+    if np.any(np.abs(s) >= 1.0):
+        raise ValueError("ramp too fast for the voltage: |sin(phi_s)| reaches %.3f" % np.abs(s).max())
+    return np.ascontiguousarray(p0c), a, np.ascontiguousarray(np.arcsin(s))
+
+
 def rf_programme(turns: int, seed: int, ring: dict = RING, ramp_to: float = 1.5,
                  mod_amplitude: float = 0.05, mod_tune_ratio: float = 0.95,
                  noise_rms: float = 1e-3):
