@@ -43,6 +43,10 @@ SMS, FP64_LANES_PER_SM = 148, 64          # B200: 2 dies x 74 SMs, 64 FP64 lanes
 CPU_SAMPLE_TURNS = 10_000                 # oracle leg: 1e9 particle-turns, about 20-25 core-seconds
 NCU_TRAFFIC_FUSED_BYTES = 1_625_344 + 570_112
 NCU_TRAFFIC_PER_TURN_BYTES = 160_020_480 + 100_925_184
+# the sec. 8(f) rows, per launch (profiles/r1_next_rows_ncu.md)
+NCU_TRAFFIC_NEXT = {"f2_fused": 2_747_904 + 388_608, "f4_per_turn": 160_019_968 + 101_635_840,
+                    "f4_histogram": 80_013_824 + 1_831_936, "f3_fused": 48_093_440 + 15_289_600,
+                    "f3_per_turn": 480_020_736 + 421_614_080}
 
 
 def measured_peaks() -> dict:
@@ -189,15 +193,17 @@ def bench_next(lt, wl, torch, stream, peaks, peak_ginstr, max_over_ranks, world,
                 t += e0.elapsed_time(e1) * 1e-3
         return max_over_ranks(t) / reps
 
-    def alu(instr, pts, sec):
+    def alu(instr, pts, sec, traffic=None):
         g = instr * pts / sec / 1e9
         return {"bound": "alu", "achieved": g, "peak": peak_ginstr, "unit": "G FP64 instr/s",
-                "frac": g / peak_ginstr, "instr_per_particle_turn": instr, "traffic": None}
+                "frac": g / peak_ginstr, "instr_per_particle_turn": instr,
+                "traffic": NCU_TRAFFIC_NEXT.get(traffic)}
 
-    def hbm(bytes_per_pt, pts, sec):
+    def hbm(bytes_per_pt, pts, sec, traffic=None):
         g = bytes_per_pt * pts / sec / 1e9
         return {"bound": "hbm", "achieved": g, "peak": hbm_peak, "unit": "GB/s",
-                "frac": g / hbm_peak, "bytes_per_particle_turn": bytes_per_pt, "traffic": None}
+                "frac": g / hbm_peak, "bytes_per_particle_turn": bytes_per_pt,
+                "traffic": NCU_TRAFFIC_NEXT.get(traffic)}
 
     out = {}
     # f2: programme, fused mode, 15 FP64 instructions per particle-turn (13 + a_t scale + psi_t add)
@@ -214,7 +220,7 @@ def bench_next(lt, wl, torch, stream, peaks, peak_ginstr, max_over_ranks, world,
     out["f2_programme_fused"] = {
         "workload": "1e5 particles x 7e4 turns, per-turn (V_t, psi_t) tables, fused mode",
         "value": world * n * turns / sec, "unit": UNIT, "ms": 1e3 * sec,
-        "roofline": alu(15, n * turns, sec)}
+        "roofline": alu(15, n * turns, sec, "f2_fused")}
     del z, d, zi, di, tr
 
     # f4: per-turn mode + 64-slice histogram of z every turn (still 32 B per particle-turn)
@@ -230,7 +236,7 @@ def bench_next(lt, wl, torch, stream, peaks, peak_ginstr, max_over_ranks, world,
     out["f4_track_slices"] = {
         "workload": "1e7 particles x 1000 turns, one launch per turn, 64-slice histogram of z per turn",
         "value": world * n * turns / sec, "unit": UNIT, "ms_per_turn": 1e3 * sec / turns,
-        "roofline": hbm(32, n * turns, sec)}
+        "roofline": hbm(32, n * turns, sec, "f4_per_turn")}
     sec = timed(lambda: tr.track_slices(z, d, n, turns, z_lo, z_hi, S, hist, mom, None, sp), 2)
     out["f4_track_slices_with_moments"] = {
         "workload": "as f4_track_slices plus moments and membership count every turn",
@@ -242,7 +248,7 @@ def bench_next(lt, wl, torch, stream, peaks, peak_ginstr, max_over_ranks, world,
     out["f4_slice_histogram"] = {
         "workload": "histogram of one state, 1e7 particles, 64 slices (8 B read per particle)",
         "value": world * n / sec, "unit": "particles/s", "ms": 1e3 * sec,
-        "roofline": hbm(8, n, sec)}
+        "roofline": hbm(8, n, sec, "f4_histogram")}
     del z, d, zs, hist, mom, tr
 
     # f3: transverse maps, fused (4 segments x 16 + 13 longitudinal FP64 instructions) and per-turn
@@ -259,7 +265,7 @@ def bench_next(lt, wl, torch, stream, peaks, peak_ginstr, max_over_ranks, world,
     out["f3_transverse_fused"] = {
         "workload": "1e6 particles x 1e4 turns, 4 segment matrices + the leap-frog turn, fused",
         "value": world * n * turns / sec, "unit": UNIT, "ms": 1e3 * sec,
-        "roofline": alu(instr, n * turns, sec)}
+        "roofline": alu(instr, n * turns, sec, "f3_fused")}
     sec = timed(lambda: tr.track_transverse_fused(co[0], co[1], co[2], co[3], None, None, n, turns, sp), 3)
     out["f3_transverse_fused_4d_only"] = {
         "workload": "as above without the longitudinal plane",
@@ -274,7 +280,7 @@ def bench_next(lt, wl, torch, stream, peaks, peak_ginstr, max_over_ranks, world,
     out["f3_transverse_per_turn"] = {
         "workload": "1e7 particles x 200 turns, one launch per turn, six arrays through HBM (480 MB)",
         "value": world * n * turns / sec, "unit": UNIT, "ms_per_turn": 1e3 * sec / turns,
-        "roofline": hbm(96, n * turns, sec)}
+        "roofline": hbm(96, n * turns, sec, "f3_per_turn")}
     del co, z, d, flush
     return out
 
