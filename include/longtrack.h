@@ -237,6 +237,35 @@ int lt_track_programme_per_turn(lt_tracker *tr, double *z_dev, double *delta_dev
                                 const double *phase_off_dev, lt_moments *moments_dev,
                                 lt_sums *sums_dev, void *stream);
 
+/* -- f2 with acceleration: energy ramp ("V, phi_s, gamma ramps per
+ *    turn from small device tables [...] gives acceleration"; G32) --------
+ * p0c_dev[0 .. turns] (device, turns + 1 doubles, eV, all > 0): the reference momentum x c BEFORE
+ * turn 1 and AFTER every turn.  volt_scale_dev / phase_off_dev as above, or NULL for a_t = 1 /
+ * psi_t = 0.  With the rest energy mc2 = p0c_eV / (beta gamma) of lt_params and, for a reference
+ * momentum p,  bg = p/mc2, beta = bg/sqrt(1 + bg^2), eta = alpha_c - 1/(1 + bg^2),
+ * A(p) = q V/(beta p), d(p) = eta C/2,  one leap-frog sub-step with factor tau that takes the
+ * reference from pb to pa is
+ *     z     -= tau d(pb) delta
+ *     delta  = (delta + tau a_t A(pb) [sin(kappa z + psi_t) + r sin(2 (kappa z + psi_t))]
+ *               - (pa - pb)/pb) * (pb/pa)
+ *     z     -= tau d(pa) delta
+ * Turn t+1 (pb = p0c[t], pa = p0c[t+1], D = pa - pb): leap-frog = sub-step(1, pb, pa);
+ * Euler-Cromer = the kick line (old z), then z -= 2 d(pa) delta; Ruth4 = sub-steps x1, x0, x1 over
+ * pb -> pb + x1 D -> (that) + x0 D -> pa.  A particle at z = 0, delta = 0 stays on the reference iff
+ * a_t A(pb) sin(psi_t) = D/pb: the caller programmes the synchronous phase through psi_t, so
+ * lt_params.phi_s must be 0 here (else LT_E_PARAM).  The tracker's own parameters are not changed
+ * by the call.  lt_track_ramp: fused multi-turn mode (17 FP64 instructions per sub-step);
+ * lt_track_ramp_per_turn: per-turn mode with the outputs of lt_track_per_turn (n_in_bucket is the
+ * stationary-bucket predicate of lt_params, whatever the ramp does).  The tables are read while
+ * the call's work runs: keep them unchanged until the stream has been synchronised. */
+int lt_track_ramp(lt_tracker *tr, double *z_dev, double *delta_dev, size_t n,
+                  unsigned long long turns, const double *p0c_dev, const double *volt_scale_dev,
+                  const double *phase_off_dev, void *stream);
+int lt_track_ramp_per_turn(lt_tracker *tr, double *z_dev, double *delta_dev, size_t n,
+                           unsigned long long turns, const double *p0c_dev,
+                           const double *volt_scale_dev, const double *phase_off_dev,
+                           lt_moments *moments_dev, lt_sums *sums_dev, void *stream);
+
 /* -- f4: longitudinal slicing at the interaction point (sec. 1.1: "the fields of
  *    the particle distribution are constructed"; the memory-bound regime;
  *    DESIGN.md G29) ---------------------------------------------------------------------------

@@ -123,17 +123,21 @@ __device__ __forceinline__ T horner(const T (&c)[N], T s) {
 //     a * A [ sin(phi_s + pi (v + p)) - sin(phi_s) + r sin(2 pi (v + p)) ],
 // a = voltage scale, p = phase offset in half periods.  PROG = 1: add p here (fast path, the
 // state is v); PROG = 2: the caller already folded p into v (exact path: v = fma(z, kappa/pi, p)).
+// PROG = 3 / 4 (energy ramp, G32): as 1 / 2, but `a` is the ABSOLUTE kick amplitude
+// tau a_t A(p_b) of the sub-step, so the unscaled polynomial sin(pi f)/f is used.
 template <typename T, int HARM, bool FQ = false, int PROG = 0>
 __device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage, T a = T(1),
                                   T p = T(0)) {
     typedef Real<T> R;
     constexpr int NS = R::NS, NC = R::NC;
-    if (PROG == 1) v = R::add(v, p);
+    static_assert(PROG < 3 || HARM != 0, "the energy ramp has no generic phi_s path");
+    const T (&sin_coef)[kMaxSin] = PROG >= 3 ? P.sin1 : P.sinA[stage];
+    if (PROG == 1 || PROG == 3) v = R::add(v, p);
     if (HARM == 1) {
         T t;
         T f = reduce_half_periods(v, &t);
         T s = R::mul(f, f);
-        T q = horner<T, NS>(P.sinA[stage], s);
+        T q = horner<T, NS>(sin_coef, s);
         if (PROG) q = R::mul(q, a);
         if (FQ) return R::fma(f, R::flip(q, t), delta);
         return R::fma(R::flip(f, t), q, delta);
@@ -141,7 +145,7 @@ __device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage
         T t;
         T f = reduce_half_periods(v, &t);
         T s = R::mul(f, f);
-        T q = horner<T, NS>(P.sinA[stage], s);   // tau A sin(pi f)/f
+        T q = horner<T, NS>(sin_coef, s);         // tau A sin(pi f)/f
         T c = horner<T, NC>(P.cos1, s);           // cos(pi f)
         if (PROG) q = R::mul(q, a);
         // sin and cos both change sign with the parity of n: flip f, and flip 2r for the cos

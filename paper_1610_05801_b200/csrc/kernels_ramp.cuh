@@ -1,0 +1,287 @@
+// kernels_ramp.cuh -- sm_100a device code for the ENERGY RAMP of SURVEY.md sec. 8(f) row f2
+// ("V, phi_s, gamma ramps per turn from small device tables"; G32).
+// CUDA path only: shares nothing with oracle/.
+//
+// The reference momentum goes p0c[t] -> p0c[t+1] over turn t+1, which makes beta, eta, the kick
+// amplitude A and the drift coefficient d functions of the turn, and re-expresses delta relative
+// to the new reference after every kick.  A turn is a sequence of SUB-STEPS (1 for leap-frog and
+// Euler-Cromer, 3 for Ruth4), each
+//     z -= db delta;   delta = g (delta + amp [sin(kappa z + psi) + r sin(2(kappa z + psi))]) + c;
+//     z -= da delta
+// with amp = tau a_t A(p_b), g = p_b/p_a, c = -(p_a - p_b)/p_a, db = tau d(p_b), da = tau d(p_a)
+// (Euler-Cromer: db = 0, da = 2 d(p_a)).  ramp_pack_kernel turns the caller's tables into one
+// 48-byte entry per sub-step; the tracking kernels are then generic in the integrator.
+#pragma once
+
+#include "kernels.cuh"
+
+namespace lt {
+
+// One sub-step, 48 bytes = three double2.
+//   exact layout (split drifts, per-turn kernel):  d0 = db, d1 = da                (metres)
+//   fast layout (merged drifts, state = phase v):  d0 = (da + db of the NEXT sub-step) kappa/pi,
+//                                                  d1 = db kappa/pi (used by the call's first sub-step)
+struct RampEntry {
+    double amp, p;      // kick amplitude; psi/pi (RF phase offset in half periods)
+    double g, c;        // delta <- g * delta + c after the kick
+    double d0, d1;
+};
+
+struct RampRing {
+    double mc2, alpha_c, qV, C;   // rest energy (eV), momentum compaction, q V (eV), circumference
+    double x1, x0;                // Ruth4 step factors
+    double to_phase, inv_pi;      // kappa/pi, 1/pi
+};
+
+__device__ __forceinline__ void ramp_ring_at(const RampRing& R, double p, double* A, double* d) {
+    const double bg = p / R.mc2;
+    const double g2 = __fma_rn(bg, bg, 1.0);
+    const double beta = bg / sqrt(g2);
+    const double eta = R.alpha_c - 1.0 / g2;
+    *A = R.qV / (beta * p);
+    *d = eta * R.C * 0.5;
+}
+
+// One thread per turn of the launch.  p0c / volt / phase are the CALL's tables (volt, phase may be
+// nullptr), t_first the absolute index of the launch's first turn, call_turns the call's length
+// (the trailing drift of the call's last sub-step is not merged with anything).
+static __global__ void ramp_pack_kernel(const double* __restrict__ p0c, const double* __restrict__ volt,
+                                 const double* __restrict__ phase, unsigned long long t_first,
+                                 unsigned int count, unsigned long long call_turns, int integ,
+                                 int fast, const __grid_constant__ RampRing R,
+                                 RampEntry* __restrict__ out) {
+    const unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    const unsigned long long T = t_first + i;
+    const double pb = p0c[T], pa = p0c[T + 1];
+    const double av = volt ? volt[T] : 1.0;
+    const double psi = phase ? phase[T] : 0.0;
+    const int nsub = integ == kRuth4 ? 3 : 1;
+    double ps[4], tau[3];
+    ps[0] = pb;
+    if (nsub == 3) {
+        const double D = pa - pb;
+        ps[1] = __fma_rn(R.x1, D, pb);
+        ps[2] = __fma_rn(R.x0, D, ps[1]);
+        ps[3] = pa;
+        tau[0] = R.x1; tau[1] = R.x0; tau[2] = R.x1;
+    } else {
+        ps[1] = pa;
+        tau[0] = 1.0;
+    }
+    double A[4], d[4];
+    for (int k = 0; k <= nsub; ++k) ramp_ring_at(R, ps[k], &A[k], &d[k]);
+    const double tau_first = integ == kEulerCromer ? 0.0 : tau[0];
+    for (int k = 0; k < nsub; ++k) {
+        RampEntry e;
+        e.amp = tau[k] * A[k] * av;
+        e.p = psi * R.inv_pi;
+        e.g = ps[k] / ps[k + 1];
+        e.c = -(ps[k + 1] - ps[k]) / ps[k + 1];
+        double db = tau[k] * d[k], da = tau[k] * d[k + 1];
+        if (integ == kEulerCromer) { db = 0.0; da = 2.0 * d[1]; }
+        if (fast) {
+            double db_next;
+            if (k + 1 < nsub) db_next = tau[k + 1] * d[k + 1];
+            else db_next = (T + 1 == call_turns) ? 0.0 : tau_first * d[nsub];
+            e.d0 = (da + db_next) * R.to_phase;
+            e.d1 = db * R.to_phase;
+        } else {
+            e.d0 = db;
+            e.d1 = da;
+        }
+        out[(size_t)i * nsub + k] = e;
+    }
+}
+
+static __global__ void ramp_advance_cursor_kernel(unsigned long long* cursor, unsigned long long by) {
+    *cursor += by;
+}
+
+// exact sub-step: state z, every drift its own FMA (bit-identical between the fused split-drift
+// kernel, the per-turn kernel and any chunking)
+template <int HARM>
+__device__ __forceinline__ void ramp_substep_exact(double& z, double& dl, const MapConsts<double>& P,
+                                                   double amp, double p, double g, double c,
+                                                   double db, double da) {
+    z = __fma_rn(-db, dl, z);
+    dl = kick<double, HARM, false, 4>(__fma_rn(z, P.to_phase, p), dl, P, 0, amp);
+    dl = __fma_rn(g, dl, c);
+    z = __fma_rn(-da, dl, z);
+}
+
+// fast sub-step: state v (phase in half periods), trailing drift merged with the next leading one.
+// 17 FP64 instructions (single harmonic): v + p, 3 reduction, f^2, 7 Horner, q * amp, kick FMA,
+// damping FMA, drift FMA.
+template <int HARM>
+__device__ __forceinline__ void ramp_substep_fast(double& v, double& dl, const MapConsts<double>& P,
+                                                  double amp, double p, double g, double c, double dm) {
+    dl = kick<double, HARM, true, 3>(v, dl, P, 0, amp, p);
+    dl = __fma_rn(g, dl, c);
+    v = __fma_rn(-dm, dl, v);
+}
+
+// `nsteps` sub-steps of one particle; tab = the item's first entry as double2[3 * nsteps]; stage =
+// the warp's private 1536-byte buffer (32 entries), refilled 32 sub-steps ahead of their use (the
+// same feed as the RF-programme kernel, kernels.cuh advance()).
+template <int HARM, bool SPLIT>
+__device__ __forceinline__ void ramp_advance(double& x, double& dl, unsigned int nsteps, int first,
+                                             int last, const MapConsts<double>& P,
+                                             const double2* __restrict__ tab,
+                                             double2* __restrict__ stage) {
+    const unsigned int lane = threadIdx.x & 31u;
+    if (!SPLIT && first) {
+        const double lead = __ldg(tab + 2).y;
+        x = __dmul_rn(x, P.to_phase);
+        x = __fma_rn(-lead, dl, x);
+    }
+    const unsigned int total2 = 3u * nsteps;
+    double2 nx[3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const unsigned int idx = lane + 32u * j;
+        nx[j] = idx < total2 ? __ldg(tab + idx) : make_double2(0.0, 0.0);
+    }
+    for (unsigned int t0 = 0; t0 < nsteps; t0 += 32) {
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < 3; ++j) stage[lane + 32u * j] = nx[j];
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const unsigned int idx = 3u * (t0 + 32u) + lane + 32u * j;
+            if (idx < total2) nx[j] = __ldg(tab + idx);
+        }
+        const unsigned int m = min(32u, nsteps - t0);
+#pragma unroll 8
+        for (unsigned int k = 0; k < m; ++k) {
+            const double2 e0 = stage[3 * k], e1 = stage[3 * k + 1], e2 = stage[3 * k + 2];
+            if (SPLIT) ramp_substep_exact<HARM>(x, dl, P, e0.x, e0.y, e1.x, e1.y, e2.x, e2.y);
+            else ramp_substep_fast<HARM>(x, dl, P, e0.x, e0.y, e1.x, e1.y, e2.x);
+        }
+    }
+    if (!SPLIT && last) x = __dmul_rn(x, P.from_phase);
+}
+
+// Fused multi-turn kernel with the ramp: the persistent ticketed work queue of
+// fused_persistent_kernel (kernels.cuh), work item = (chunk of item_steps sub-steps) x (32 particles).
+template <int HARM, bool SPLIT>
+__global__ void __launch_bounds__(1024, 1)
+ramp_persistent_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, size_t n,
+                       unsigned int nsteps, unsigned int item_steps, int first_launch, int last_launch,
+                       int dynamic, unsigned long long* __restrict__ ticket,
+                       unsigned int* __restrict__ done, const __grid_constant__ MapConsts<double> P,
+                       const double2* __restrict__ table) {
+    extern __shared__ __align__(16) unsigned char ramp_smem[];   // 1536 B per warp + residency cap
+    const unsigned int lane = threadIdx.x & 31u;
+    const unsigned long long groups = (n + 31) / 32;
+    const unsigned int nchunks = (nsteps + item_steps - 1) / item_steps;
+    const unsigned long long total = groups * nchunks;
+    const unsigned long long slots = (unsigned long long)gridDim.x * (blockDim.x >> 5);
+    unsigned long long next = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
+    double2* stage = reinterpret_cast<double2*>(ramp_smem) + 96u * (threadIdx.x >> 5);
+    for (;;) {
+        unsigned long long t = next;
+        if (dynamic) {
+            if (lane == 0) t = atomicAdd(ticket, 1ULL);
+            t = __shfl_sync(0xffffffffu, t, 0);
+        } else {
+            next += slots;
+        }
+        if (t >= total) break;
+        const unsigned int c = (unsigned int)(t / groups);
+        const unsigned long long g = t - (unsigned long long)c * groups;
+        if (c > 0) {
+            while (ld_acquire_u32(done + g) < c) __nanosleep(64);
+        }
+        const size_t i = (size_t)g * 32 + lane;
+        double x = (i < n) ? __ldcg(z_arr + i) : 0.0;
+        double dl = (i < n) ? __ldcg(d_arr + i) : 0.0;
+        const int first = first_launch && c == 0;
+        const int last = last_launch && c == nchunks - 1;
+        const unsigned int ns = (c == nchunks - 1) ? nsteps - c * item_steps : item_steps;
+        ramp_advance<HARM, SPLIT>(x, dl, ns, first, last, P, table + 3 * (size_t)c * item_steps, stage);
+        if (i < n) { __stcg(z_arr + i, x); __stcg(d_arr + i, dl); }
+        if (nchunks > 1) {
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) st_release_u32(done + g, c + 1);
+        }
+    }
+}
+
+// Per-turn mode with the ramp: the structure of per_turn_kernel (persistent CTAs, double2 tiles,
+// all loads of a tile before its arithmetic, moments fused, sweep direction alternating), the
+// turn's NSUB entries read once per thread from the packed table at turn *cursor + k.
+template <int HARM, int NSUB, bool MOMENTS, bool VEC, int UNR>
+__global__ void ramp_per_turn_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, size_t n,
+                                     int reverse, double* __restrict__ partials,
+                                     const __grid_constant__ MapConsts<double> P,
+                                     const RampEntry* __restrict__ table,
+                                     const unsigned long long* __restrict__ cursor, int k) {
+    RampEntry e[NSUB];
+    {
+        const double2* src = reinterpret_cast<const double2*>(table + (*cursor + (unsigned long long)k) * NSUB);
+#pragma unroll
+        for (int s = 0; s < NSUB; ++s) {
+            const double2 a = __ldg(src + 3 * s), b = __ldg(src + 3 * s + 1), c = __ldg(src + 3 * s + 2);
+            e[s].amp = a.x; e[s].p = a.y; e[s].g = b.x; e[s].c = b.y; e[s].d0 = c.x; e[s].d1 = c.y;
+        }
+    }
+    auto turn = [&](double& z, double& dl) {
+#pragma unroll
+        for (int s = 0; s < NSUB; ++s)
+            ramp_substep_exact<HARM>(z, dl, P, e[s].amp, e[s].p, e[s].g, e[s].c, e[s].d0, e[s].d1);
+    };
+    Sums acc;
+    acc.zero();
+    if (VEC) {
+        const size_t npair = n >> 1;
+        const size_t tile_pairs = (size_t)blockDim.x * UNR;
+        const size_t ntiles = (npair + tile_pairs - 1) / tile_pairs;
+        for (size_t tl = blockIdx.x; tl < ntiles; tl += gridDim.x) {
+            const size_t tix = reverse ? (ntiles - 1 - tl) : tl;
+            const size_t base = tix * tile_pairs;
+            double2 a[UNR], b[UNR];
+#pragma unroll
+            for (int u = 0; u < UNR; ++u) {
+                const size_t p = base + (size_t)u * blockDim.x + threadIdx.x;
+                if (p < npair) {
+                    a[u] = reinterpret_cast<const double2*>(z_arr)[p];
+                    b[u] = reinterpret_cast<const double2*>(d_arr)[p];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < UNR; ++u) {
+                const size_t p = base + (size_t)u * blockDim.x + threadIdx.x;
+                if (p < npair) {
+                    turn(a[u].x, b[u].x);
+                    turn(a[u].y, b[u].y);
+                    reinterpret_cast<double2*>(z_arr)[p] = a[u];
+                    reinterpret_cast<double2*>(d_arr)[p] = b[u];
+                    if (MOMENTS) {
+                        acc.add(a[u].x, b[u].x, in_bucket<double>(a[u].x, b[u].x, P));
+                        acc.add(a[u].y, b[u].y, in_bucket<double>(a[u].y, b[u].y, P));
+                    }
+                }
+            }
+        }
+        if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+            double zz = z_arr[n - 1], dd = d_arr[n - 1];
+            turn(zz, dd);
+            z_arr[n - 1] = zz; d_arr[n - 1] = dd;
+            if (MOMENTS) acc.add(zz, dd, in_bucket<double>(zz, dd, P));
+        }
+    } else {
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+             i += (size_t)gridDim.x * blockDim.x) {
+            double zz = z_arr[i], dd = d_arr[i];
+            turn(zz, dd);
+            z_arr[i] = zz; d_arr[i] = dd;
+            if (MOMENTS) acc.add(zz, dd, in_bucket<double>(zz, dd, P));
+        }
+    }
+    if (MOMENTS) block_reduce_store(acc, partials + (size_t)blockIdx.x * kPartialStride);
+}
+
+}  // namespace lt

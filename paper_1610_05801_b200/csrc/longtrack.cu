@@ -638,6 +638,7 @@ int lt_destroy(lt_tracker* tr) {
     if (tr->stage_count) cudaFree(tr->stage_count);
     if (tr->own_stream) cudaStreamDestroy(tr->own_stream);
     destroy_next(tr);
+    destroy_ramp(tr);
     (void)cudaGetLastError();
     delete tr;
     return LT_OK;

@@ -1,0 +1,243 @@
+// longtrack_ramp.cu -- host side of lt_track_ramp / lt_track_ramp_per_turn: the energy ramp of
+// SURVEY.md sec. 8(f) row f2 (G32).
+// CUDA path only: nothing here includes, links or calls anything under oracle/.
+#include "tracker.hpp"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "kernels_ramp.cuh"
+
+using namespace lt;
+using namespace lt_host;
+
+namespace {
+
+constexpr unsigned long long kRampChunkMax = 1ULL << 18;   // turns packed per fused launch
+
+int nsub_of(const lt_tracker* tr) { return tr->p.integrator == LT_RUTH4 ? 3 : 1; }
+
+RampRing make_ring(const lt_tracker* tr) {
+    RampRing R;
+    const long double gamma = tr->p.gamma;
+    const long double beta = sqrtl(1.0L - 1.0L / (gamma * gamma));
+    R.mc2 = (double)((long double)tr->p.p0c_eV / (beta * gamma));
+    R.alpha_c = tr->p.alpha_c;
+    R.qV = tr->p.charge_e * tr->p.voltage_V;
+    R.C = tr->p.circumference_m;
+    const long double w = cbrtl(2.0L);
+    R.x1 = (double)(1.0L / (2.0L - w));
+    R.x0 = (double)(-w / (2.0L - w));
+    R.to_phase = tr->c64.to_phase;
+    R.inv_pi = 0.31830988618379067154;
+    return R;
+}
+
+int ensure_ramp_table(lt_tracker* tr, size_t entries) {
+    if (tr->ramp_entries >= entries) return LT_OK;
+    if (tr->ramp_table) { LT_CUDA(tr, cudaFree(tr->ramp_table)); tr->ramp_table = nullptr; tr->ramp_entries = 0; }
+    LT_CUDA(tr, cudaMalloc(&tr->ramp_table, entries * sizeof(RampEntry)));
+    tr->ramp_entries = entries;
+    return LT_OK;
+}
+
+int check_args(const lt_tracker* tr, const double* z, const double* d, size_t n,
+               unsigned long long turns, const double* p0c, const double* volt, const double* phase) {
+    if (!tr) return LT_E_NULL;
+    if (tr->harm == 0) return LT_E_PARAM;               // phi_s != 0: programme psi_t instead (G32)
+    if (n == 0 || turns == 0) return LT_OK;
+    if (!z || !d || !p0c) return LT_E_NULL;
+    if (!aligned(z, 8) || !aligned(d, 8) || !aligned(p0c, 8)) return LT_E_ALIGN;
+    if ((volt && !aligned(volt, 8)) || (phase && !aligned(phase, 8))) return LT_E_ALIGN;
+    if (n > ((size_t)1 << 40)) return LT_E_PARAM;
+    return LT_OK;
+}
+
+template <int HARM, bool SPLIT>
+cudaError_t launch_ramp_fused(double* z, double* d, size_t n, unsigned int nsteps, unsigned int item_steps,
+                              int first, int last, const PersistentPlan& pl, const lt_tracker* tr,
+                              cudaStream_t st) {
+    auto kern = ramp_persistent_kernel<HARM, SPLIT>;
+    // 1 CTA/SM: > half of the 227 KB; 2 CTAs/SM: > a third (and >= 1536 B per warp of staging)
+    const int smem = pl.ctas_per_sm == 1 ? 120 * 1024 : 80 * 1024;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    kern<<<tr->sm_count * pl.ctas_per_sm, pl.threads, smem, st>>>(
+        z, d, n, nsteps, item_steps, first, last, pl.dynamic, tr->sched,
+        reinterpret_cast<unsigned int*>(tr->sched + 1), tr->c64,
+        reinterpret_cast<const double2*>(tr->ramp_table));
+    return cudaGetLastError();
+}
+
+template <int HARM, int NSUB>
+cudaError_t launch_ramp_turn(double* z, double* d, size_t n, int reverse, double* partials, bool moments,
+                             bool vec, int grid, const lt_tracker* tr, int k, cudaStream_t st) {
+    const RampEntry* tab = reinterpret_cast<const RampEntry*>(tr->ramp_table);
+#define LT_RT(M, V) ramp_per_turn_kernel<HARM, NSUB, M, V, kPerTurnUnroll><<<grid, kPerTurnThreads, 0, st>>>( \
+        z, d, n, reverse, partials, tr->c64, tab, tr->cursor, k)
+    if (moments) { if (vec) LT_RT(true, true); else LT_RT(true, false); }
+    else         { if (vec) LT_RT(false, true); else LT_RT(false, false); }
+#undef LT_RT
+    return cudaGetLastError();
+}
+
+cudaError_t enqueue_ramp_batch(lt_tracker* tr, double* z, double* d, size_t n, unsigned long long t0,
+                               int nb, bool moments, lt_moments* mo, lt_sums* so, bool vec, int grid,
+                               cudaStream_t st) {
+    const int nsub = nsub_of(tr);
+    for (int k = 0; k < nb; ++k) {
+        const int reverse = tr->per_turn_reverse ? (int)((t0 + k) & 1ULL) : 0;
+        double* part = tr->partials + (size_t)k * grid * kPartialStride;
+        cudaError_t e;
+        if (tr->harm == 1)
+            e = nsub == 3 ? launch_ramp_turn<1, 3>(z, d, n, reverse, part, moments, vec, grid, tr, k, st)
+                          : launch_ramp_turn<1, 1>(z, d, n, reverse, part, moments, vec, grid, tr, k, st);
+        else
+            e = nsub == 3 ? launch_ramp_turn<2, 3>(z, d, n, reverse, part, moments, vec, grid, tr, k, st)
+                          : launch_ramp_turn<2, 1>(z, d, n, reverse, part, moments, vec, grid, tr, k, st);
+        if (e != cudaSuccess) return e;
+        tr->launches++;
+    }
+    if (moments)
+        finalize_kernel<<<nb, 256, 0, st>>>(tr->partials, grid, n, tr->cursor,
+                                            reinterpret_cast<unsigned int*>(tr->cursor + 1),
+                                            reinterpret_cast<MomentsOut*>(mo),
+                                            reinterpret_cast<SumsOut*>(so), nullptr);
+    else
+        ramp_advance_cursor_kernel<<<1, 1, 0, st>>>(tr->cursor, (unsigned long long)nb);
+    tr->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+namespace lt_host {
+void destroy_ramp(lt_tracker* tr) {
+    if (tr->ramp_table) cudaFree(tr->ramp_table);
+    tr->ramp_table = nullptr;
+    tr->ramp_entries = 0;
+}
+}  // namespace lt_host
+
+extern "C" {
+
+int lt_track_ramp(lt_tracker* tr, double* z, double* d, size_t n, unsigned long long turns,
+                  const double* p0c, const double* volt, const double* phase, void* stream) {
+    int rc = check_args(tr, z, d, n, turns, p0c, volt, phase);
+    if (rc || n == 0 || turns == 0) return rc;
+    rc = ensure_device(tr);
+    if (rc) return rc;
+    rc = ensure_sched(tr, n);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int nsub = nsub_of(tr);
+    const bool split = tr->split_drifts != 0;
+    const unsigned long long chunk_max =
+        std::min<unsigned long long>((unsigned long long)tr->chunk_turns, kRampChunkMax);
+    rc = ensure_ramp_table(tr, (size_t)std::min<unsigned long long>(turns, chunk_max) * nsub);
+    if (rc) return rc;
+    const PersistentPlan pl = plan_persistent(tr, n, turns);
+    const RampRing R = make_ring(tr);
+    unsigned long long done = 0;
+    while (done < turns) {
+        const unsigned long long chunk = std::min<unsigned long long>(turns - done, chunk_max);
+        const int first = done == 0, last = done + chunk == turns;
+        const unsigned int item_turns =
+            pl.dynamic ? std::min<unsigned int>(pl.item_turns, (unsigned int)chunk) : (unsigned int)chunk;
+        // the table of the previous chunk is free again: its kernel precedes this one on the stream
+        ramp_pack_kernel<<<(unsigned)((chunk + 255) / 256), 256, 0, st>>>(
+            p0c, volt, phase, done, (unsigned int)chunk, turns, tr->p.integrator, split ? 0 : 1, R,
+            reinterpret_cast<RampEntry*>(tr->ramp_table));
+        LT_CUDA(tr, cudaGetLastError());
+        if (pl.dynamic) LT_CUDA(tr, cudaMemsetAsync(tr->sched, 0, 8 + 4 * ((n + 31) / 32), st));
+        const unsigned int nsteps = (unsigned int)chunk * nsub, item_steps = item_turns * nsub;
+        cudaError_t e;
+        if (tr->harm == 1)
+            e = split ? launch_ramp_fused<1, true>(z, d, n, nsteps, item_steps, first, last, pl, tr, st)
+                      : launch_ramp_fused<1, false>(z, d, n, nsteps, item_steps, first, last, pl, tr, st);
+        else
+            e = split ? launch_ramp_fused<2, true>(z, d, n, nsteps, item_steps, first, last, pl, tr, st)
+                      : launch_ramp_fused<2, false>(z, d, n, nsteps, item_steps, first, last, pl, tr, st);
+        LT_CUDA(tr, e);
+        tr->launches += 2;
+        done += chunk;
+    }
+    tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
+    tr->last_block = pl.threads;
+    tr->last_ilp = 1;
+    tr->last_mode = pl.dynamic ? 3 : 2;
+    tr->last_item_turns = pl.dynamic ? pl.item_turns : 0;
+    return LT_OK;
+}
+
+int lt_track_ramp_per_turn(lt_tracker* tr, double* z, double* d, size_t n, unsigned long long turns,
+                           const double* p0c, const double* volt, const double* phase,
+                           lt_moments* mo, lt_sums* so, void* stream) {
+    int rc = check_args(tr, z, d, n, turns, p0c, volt, phase);
+    if (rc || n == 0 || turns == 0) return rc;
+    if ((mo && !aligned(mo, 8)) || (so && !aligned(so, 8))) return LT_E_ALIGN;
+    if (turns > (1ULL << 26)) return LT_E_PARAM;         // the whole call's table is packed at once
+    rc = ensure_device(tr);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int nsub = nsub_of(tr);
+    rc = ensure_ramp_table(tr, (size_t)turns * nsub);
+    if (rc) return rc;
+    const bool moments = mo || so;
+    const bool vec = aligned(z, 16) && aligned(d, 16);
+    const int grid = per_turn_grid(tr, n);
+    rc = ensure_scratch(tr, grid);
+    if (rc) return rc;
+    const RampRing R = make_ring(tr);
+    for (unsigned long long off = 0; off < turns; off += 1ULL << 20) {
+        const unsigned int cnt = (unsigned int)std::min<unsigned long long>(1ULL << 20, turns - off);
+        ramp_pack_kernel<<<(cnt + 255) / 256, 256, 0, st>>>(
+            p0c, volt, phase, off, cnt, turns, tr->p.integrator, 0, R,
+            reinterpret_cast<RampEntry*>(tr->ramp_table) + (size_t)off * nsub);
+        LT_CUDA(tr, cudaGetLastError());
+        tr->launches++;
+    }
+    set_cursor_kernel<<<1, 1, 0, st>>>(tr->cursor, reinterpret_cast<unsigned int*>(tr->cursor + 1), 0ULL);
+    LT_CUDA(tr, cudaGetLastError());
+    tr->launches++;
+    unsigned long long t0 = 0;
+    if (tr->per_turn_graph && turns >= 2ULL * kBatchTurns) {
+        GraphKey key;
+        std::memset(&key, 0, sizeof(key));
+        key.z = z; key.d = d; key.moments = mo; key.sums = so; key.n = n;
+        key.reverse = (int)tr->per_turn_reverse; key.grid = grid;
+        key.ramp = tr->ramp_table; key.nsub = nsub;
+        if (!tr->graph_exec || !(tr->graph_key == key)) {
+            if (tr->graph_exec) { cudaGraphExecDestroy(tr->graph_exec); tr->graph_exec = nullptr; }
+            if (!tr->capture_stream)
+                LT_CUDA(tr, cudaStreamCreateWithFlags(&tr->capture_stream, cudaStreamNonBlocking));
+            cudaGraph_t graph = nullptr;
+            LT_CUDA(tr, cudaStreamBeginCapture(tr->capture_stream, cudaStreamCaptureModeThreadLocal));
+            const long long before = tr->launches;
+            cudaError_t e = enqueue_ramp_batch(tr, z, d, n, 0, kBatchTurns, moments, mo, so, vec, grid,
+                                               tr->capture_stream);
+            tr->launches = before;      // capture enqueues nothing
+            cudaError_t e2 = cudaStreamEndCapture(tr->capture_stream, &graph);
+            LT_CUDA(tr, e);
+            LT_CUDA(tr, e2);
+            cudaError_t e3 = cudaGraphInstantiate(&tr->graph_exec, graph, 0);
+            cudaGraphDestroy(graph);
+            LT_CUDA(tr, e3);
+            tr->graph_key = key;
+        }
+        while (turns - t0 >= (unsigned long long)kBatchTurns) {
+            LT_CUDA(tr, cudaGraphLaunch(tr->graph_exec, st));
+            tr->launches += kBatchTurns + 1;
+            t0 += kBatchTurns;
+        }
+    }
+    while (t0 < turns) {
+        const int nb = (int)std::min<unsigned long long>(kBatchTurns, turns - t0);
+        LT_CUDA(tr, enqueue_ramp_batch(tr, z, d, n, t0, nb, moments, mo, so, vec, grid, st));
+        t0 += nb;
+    }
+    return LT_OK;
+}
+
+}  // extern "C"

@@ -27,11 +27,13 @@ struct GraphKey {
     void* hist;
     double z_lo, z_hi;
     int n_slices;
+    const void* ramp;         // energy ramp: the packed table baked into the captured launches
+    int nsub;
     bool operator==(const GraphKey& o) const {
         return z == o.z && d == o.d && moments == o.moments && sums == o.sums && n == o.n &&
                f32 == o.f32 && reverse == o.reverse && grid == o.grid && volt == o.volt &&
                phase == o.phase && hist == o.hist && z_lo == o.z_lo && z_hi == o.z_hi &&
-               n_slices == o.n_slices;
+               n_slices == o.n_slices && ramp == o.ramp && nsub == o.nsub;
     }
 };
 
@@ -74,6 +76,9 @@ struct lt_tracker {
     // f2: packed programme table of the current fused chunk
     double2* prog_table;
     size_t prog_entries;
+    // f2 with acceleration: packed sub-step entries (lt::RampEntry, 48 B each)
+    void* ramp_table;
+    size_t ramp_entries;
     // f3: lattice
     double* lattice_host;     // [n_seg][16], row-major
     double* lattice_dev;
@@ -106,5 +111,6 @@ cudaError_t launch_per_turn_f64(const lt_tracker* tr, double* z, double* d, size
                                 double* partials, bool moments, bool vec_ok, int grid,
                                 cudaStream_t st);
 void destroy_next(lt_tracker* tr);       // frees what longtrack_next.cu allocated
+void destroy_ramp(lt_tracker* tr);       // frees what longtrack_ramp.cu allocated
 
 }  // namespace lt_host

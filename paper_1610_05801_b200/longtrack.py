@@ -92,6 +92,8 @@ def _load():
         # SURVEY.md sec. 8(f) rows f2-f4
         "lt_track_programme": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp]),
         "lt_track_programme_per_turn": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp, vp, vp]),
+        "lt_track_ramp": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp, vp]),
+        "lt_track_ramp_per_turn": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp, vp, vp, vp]),
         "lt_slice_histogram": (c_int, [vp, vp, sz, c_double, c_double, c_int, vp, vp]),
         "lt_track_slices": (c_int, [vp, vp, vp, sz, ull, c_double, c_double, c_int, vp, vp, vp,
                                     vp]),
@@ -208,6 +210,18 @@ class Tracker:
         self._check(_lib.lt_track_programme_per_turn(self._h, _ptr(z), _ptr(delta), n, turns,
                                                      _ptr(volt_scale), _ptr(phase_off),
                                                      _ptr(moments), _ptr(sums), stream))
+
+    def track_ramp(self, z, delta, n: int, turns: int, p0c, volt_scale=None, phase_off=None,
+                   stream: int = 0):
+        """Energy ramp (G32): p0c has turns + 1 entries; the two tables may be None."""
+        self._check(_lib.lt_track_ramp(self._h, _ptr(z), _ptr(delta), n, turns, _ptr(p0c),
+                                       _ptr(volt_scale), _ptr(phase_off), stream))
+
+    def track_ramp_per_turn(self, z, delta, n: int, turns: int, p0c, volt_scale=None,
+                            phase_off=None, moments=None, sums=None, stream: int = 0):
+        self._check(_lib.lt_track_ramp_per_turn(self._h, _ptr(z), _ptr(delta), n, turns,
+                                                _ptr(p0c), _ptr(volt_scale), _ptr(phase_off),
+                                                _ptr(moments), _ptr(sums), stream))
 
     def slice_histogram(self, z, n: int, z_lo: float, z_hi: float, n_slices: int, hist,
                         stream: int = 0):

@@ -145,6 +145,10 @@ NEXT_CONFIGS = dict(
     # "parameter changes of the accelerator setting" switched on
     f2_programme=dict(name="f2_programme", n=100_000, turns=70_000, integrator="leapfrog",
                       ratio2=0.0, dist="gauss", sigma_z=0.23, seed=16110, programme_seed=16120),
+    # f2 with acceleration ("gamma ramps per turn"; G32): the same
+    # run shape, reference momentum 26 -> 60 GeV/c on the synchronous phase (`energy_ramp`)
+    f2_ramp=dict(name="f2_ramp", n=100_000, turns=70_000, integrator="leapfrog", ratio2=0.0,
+                 dist="gauss", sigma_z=0.08, seed=16113, p_start=26e9, p_end=60e9),
     # f3: "the same matrix is repeatedly acting on the typically 10^5 to 10^7 macro-particles'
     # state vectors"
     f3_transverse=dict(name="f3_transverse", n=1_000_000, turns=10_000, n_seg=4, seed=16111,

@@ -139,6 +139,15 @@ def test_next_rows_validate_arguments_before_touching_a_device(lt):
     assert code(tr.track_programme, buf, buf, 8, 4, None, buf) == lt.E_NULL
     assert code(tr.track_programme_per_turn, buf, buf, 8, 4, buf, None) == lt.E_NULL
     assert code(tr.track_programme, buf, buf, 0, 4, None, None) == 0           # n == 0: no-op
+    # f2 with the energy ramp: p0c is required, the other two tables are optional, phi_s must be 0
+    assert code(tr.track_ramp, buf, buf, 8, 4, None) == lt.E_NULL
+    assert code(tr.track_ramp_per_turn, buf, buf, 8, 4, None, buf, buf) == lt.E_NULL
+    assert code(tr.track_ramp, buf, buf, 0, 4, None) == 0                      # n == 0: no-op
+    assert code(tr.track_ramp, buf, buf, 8, 0, None) == 0                      # zero turns: no-op
+    assert code(lt.Tracker(wl.RING, "leapfrog", 0.0, 0.3).track_ramp, buf, buf, 8, 4, buf) == lt.E_PARAM
+    if not torch.cuda.is_available():
+        assert code(tr.track_ramp, buf, buf, 8, 4, buf) == lt.E_CUDA
+        assert code(tr.track_ramp_per_turn, buf, buf, 8, 4, buf) == lt.E_CUDA
     # f3: the lattice
     four = (buf, buf, buf, buf)
     assert code(tr.track_transverse_fused, *four, None, None, 8, 4) == lt.E_PARAM   # none set
