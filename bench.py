@@ -223,6 +223,36 @@ def bench_next(lt, wl, torch, stream, peaks, peak_ginstr, max_over_ranks, world,
         "roofline": alu(15, n * turns, sec, "f2_fused")}
     del z, d, zi, di, tr
 
+    # f2 with acceleration: energy ramp 26 -> 60 GeV/c, 17 FP64 instructions per particle-turn
+    # (13 + psi_t add + amplitude scale + damping FMA + the drift coefficient from the table)
+    c = wl.NEXT_CONFIGS["f2_ramp"]
+    n, turns = c["n"], c["turns"]
+    z0, d0 = wl.gaussian_bunch(n, c["sigma_z"], c["seed"] + rank)
+    p0c, a, psi = wl.energy_ramp(turns, c["p_start"], c["p_end"])
+    z, d = torch.from_numpy(z0).cuda(), torch.from_numpy(d0).cuda()
+    zi, di = z.clone(), d.clone()
+    pc, at, pt = (torch.from_numpy(v).cuda() for v in (p0c, a, psi))
+    tr = lt.Tracker(wl.RING, "leapfrog")
+    sec = timed(lambda: tr.track_ramp(z, d, n, turns, pc, at, pt, sp), 5,
+                lambda: (z.copy_(zi), d.copy_(di)))
+    out["f2_ramp_fused"] = {
+        "workload": "1e5 particles x 7e4 turns, reference momentum 26 -> 60 GeV/c on the synchronous phase, fused mode",
+        "value": world * n * turns / sec, "unit": UNIT, "ms": 1e3 * sec,
+        "roofline": alu(17, n * turns, sec)}
+    del z, d, zi, di, tr
+    c3 = wl.CONFIGS[3]
+    n, turns = c3["n"], 256
+    z0, d0 = wl.gaussian_bunch(n, 0.08, c["seed"] + 1 + rank)
+    z, d = torch.from_numpy(z0).cuda(), torch.from_numpy(d0).cuda()
+    mom = torch.zeros(turns * lt.MOMENTS_DTYPE.itemsize, dtype=torch.uint8, device="cuda")
+    tr = lt.Tracker(wl.RING, "leapfrog")
+    sec = timed(lambda: tr.track_ramp_per_turn(z, d, n, turns, pc, at, pt, mom, None, sp), 2)
+    out["f2_ramp_per_turn"] = {
+        "workload": "1e7 particles x 256 turns of the same ramp, one launch per turn, moments every turn",
+        "value": world * n * turns / sec, "unit": UNIT, "ms_per_turn": 1e3 * sec / turns,
+        "roofline": hbm(32, n * turns, sec)}
+    del z, d, mom, tr, pc, at, pt
+
     # f4: per-turn mode + 64-slice histogram of z every turn (still 32 B per particle-turn)
     c = wl.NEXT_CONFIGS["f4_slices"]
     n, turns = c["n"], c["turns"]
