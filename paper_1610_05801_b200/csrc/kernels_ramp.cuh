@@ -121,44 +121,53 @@ __device__ __forceinline__ void ramp_substep_fast(double& v, double& dl, const M
     v = __fma_rn(-dm, dl, v);
 }
 
+__device__ __forceinline__ void cp_async_16(void* smem_dst, const void* gmem_src) {
+    const unsigned int dst = (unsigned int)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+
 // `nsteps` sub-steps of one particle; tab = the item's first entry as double2[3 * nsteps]; stage =
-// the warp's private 1536-byte buffer (32 entries), refilled 32 sub-steps ahead of their use (the
-// same feed as the RF-programme kernel, kernels.cuh advance()).
+// the warp's private double buffer in shared memory (2 x 32 entries = 3072 B).  While the warp
+// works through one block of 32 entries, the next block arrives by cp.async (no registers held,
+// no L2 latency on the dependent FP64 chain; a per-sub-step global load stalled the RF-programme
+// kernel once per 128-byte line, profiles/r1_next_rows_ncu.md).
 template <int HARM, bool SPLIT>
 __device__ __forceinline__ void ramp_advance(double& x, double& dl, unsigned int nsteps, int first,
                                              int last, const MapConsts<double>& P,
                                              const double2* __restrict__ tab,
                                              double2* __restrict__ stage) {
     const unsigned int lane = threadIdx.x & 31u;
+    const unsigned int total2 = 3u * nsteps;
+    auto fetch = [&](unsigned int t0, unsigned int buf) {
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const unsigned int idx = 3u * t0 + lane + 32u * j;
+            if (idx < total2) cp_async_16(stage + 96u * buf + lane + 32u * j, tab + idx);
+        }
+        cp_async_commit();
+    };
+    fetch(0, 0);
     if (!SPLIT && first) {
         const double lead = __ldg(tab + 2).y;
         x = __dmul_rn(x, P.to_phase);
         x = __fma_rn(-lead, dl, x);
     }
-    const unsigned int total2 = 3u * nsteps;
-    double2 nx[3];
-#pragma unroll
-    for (int j = 0; j < 3; ++j) {
-        const unsigned int idx = lane + 32u * j;
-        nx[j] = idx < total2 ? __ldg(tab + idx) : make_double2(0.0, 0.0);
-    }
-    for (unsigned int t0 = 0; t0 < nsteps; t0 += 32) {
+    unsigned int buf = 0;
+    for (unsigned int t0 = 0; t0 < nsteps; t0 += 32, buf ^= 1u) {
+        fetch(t0 + 32u, buf ^ 1u);           // the block after this one (an empty group at the end)
+        cp_async_wait_1();                   // this block has landed
         __syncwarp();
-#pragma unroll
-        for (int j = 0; j < 3; ++j) stage[lane + 32u * j] = nx[j];
-        __syncwarp();
-#pragma unroll
-        for (int j = 0; j < 3; ++j) {
-            const unsigned int idx = 3u * (t0 + 32u) + lane + 32u * j;
-            if (idx < total2) nx[j] = __ldg(tab + idx);
-        }
+        const double2* __restrict__ cur = stage + 96u * buf;
         const unsigned int m = min(32u, nsteps - t0);
 #pragma unroll 8
         for (unsigned int k = 0; k < m; ++k) {
-            const double2 e0 = stage[3 * k], e1 = stage[3 * k + 1], e2 = stage[3 * k + 2];
+            const double2 e0 = cur[3 * k], e1 = cur[3 * k + 1], e2 = cur[3 * k + 2];
             if (SPLIT) ramp_substep_exact<HARM>(x, dl, P, e0.x, e0.y, e1.x, e1.y, e2.x, e2.y);
             else ramp_substep_fast<HARM>(x, dl, P, e0.x, e0.y, e1.x, e1.y, e2.x);
         }
+        __syncwarp();                        // all lanes are done with `buf` before it is refilled
     }
     if (!SPLIT && last) x = __dmul_rn(x, P.from_phase);
 }
@@ -172,14 +181,14 @@ ramp_persistent_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, s
                        int dynamic, unsigned long long* __restrict__ ticket,
                        unsigned int* __restrict__ done, const __grid_constant__ MapConsts<double> P,
                        const double2* __restrict__ table) {
-    extern __shared__ __align__(16) unsigned char ramp_smem[];   // 1536 B per warp + residency cap
+    extern __shared__ __align__(16) unsigned char ramp_smem[];   // 3072 B per warp + residency cap
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned long long groups = (n + 31) / 32;
     const unsigned int nchunks = (nsteps + item_steps - 1) / item_steps;
     const unsigned long long total = groups * nchunks;
     const unsigned long long slots = (unsigned long long)gridDim.x * (blockDim.x >> 5);
     unsigned long long next = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
-    double2* stage = reinterpret_cast<double2*>(ramp_smem) + 96u * (threadIdx.x >> 5);
+    double2* stage = reinterpret_cast<double2*>(ramp_smem) + 192u * (threadIdx.x >> 5);
     for (;;) {
         unsigned long long t = next;
         if (dynamic) {
