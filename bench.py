@@ -46,7 +46,8 @@ NCU_TRAFFIC_PER_TURN_BYTES = 160_020_480 + 100_925_184
 # the sec. 8(f) rows, per launch (profiles/r1_next_rows_ncu.md)
 NCU_TRAFFIC_NEXT = {"f2_fused": 2_747_904 + 388_608, "f4_per_turn": 160_019_968 + 101_635_840,
                     "f4_histogram": 80_013_824 + 1_831_936, "f3_fused": 48_093_440 + 15_289_600,
-                    "f3_per_turn": 480_020_736 + 421_614_080}
+                    "f3_per_turn": 480_020_736 + 421_614_080,
+                    "f2_ramp_fused": 4_984_576 + 154_880, "f2_ramp_per_turn": 160_047_104 + 101_511_424}
 
 
 def measured_peaks() -> dict:
@@ -238,7 +239,7 @@ def bench_next(lt, wl, torch, stream, peaks, peak_ginstr, max_over_ranks, world,
     out["f2_ramp_fused"] = {
         "workload": "1e5 particles x 7e4 turns, reference momentum 26 -> 60 GeV/c on the synchronous phase, fused mode",
         "value": world * n * turns / sec, "unit": UNIT, "ms": 1e3 * sec,
-        "roofline": alu(17, n * turns, sec)}
+        "roofline": alu(17, n * turns, sec, "f2_ramp_fused")}
     del z, d, zi, di, tr
     c3 = wl.CONFIGS[3]
     n, turns = c3["n"], 256
@@ -250,7 +251,7 @@ def bench_next(lt, wl, torch, stream, peaks, peak_ginstr, max_over_ranks, world,
     out["f2_ramp_per_turn"] = {
         "workload": "1e7 particles x 256 turns of the same ramp, one launch per turn, moments every turn",
         "value": world * n * turns / sec, "unit": UNIT, "ms_per_turn": 1e3 * sec / turns,
-        "roofline": hbm(32, n * turns, sec)}
+        "roofline": hbm(32, n * turns, sec, "f2_ramp_per_turn")}
     del z, d, mom, tr, pc, at, pt
 
     # f4: per-turn mode + 64-slice histogram of z every turn (still 32 B per particle-turn)

@@ -110,6 +110,23 @@ def test_programme_split_drift_fused_equals_per_turn_bits_and_chunking_is_invisi
     assert np.array_equal(zs, zt) and np.array_equal(ds, dt)
 
 
+@pytest.mark.parametrize("turns", [1, 2, 31, 32, 33, 64, 65, 97])
+def test_programme_call_lengths_around_the_staging_block(turns):
+    """The fused kernel stages the table in blocks of 32 entries per warp and peels the call's
+    last turn: lengths around the block size, merged and split drifts, all integrators."""
+    a, psi = strong_programme(turns, seed=70 + turns)
+    for integrator in INTEGRATORS:
+        tr, p = both(integrator, 0.5)
+        z0, d0 = wl.gaussian_bunch(777, 0.23, 27, ratio2=0.5)
+        zo, do = oracle.track_programme(p, z0, d0, a, psi)
+        for split in (0, 1):
+            tr.set_option(lt.OPT_SPLIT_DRIFTS, split)
+            zg, dg = gpu_programme(tr, z0, d0, a, psi, "fused")
+            g = oracle.derive(p)
+            assert np.abs(zg - zo).max() / g["z_max"] <= 1e-11, (integrator, split)
+            assert np.abs(dg - do).max() / wl.matched_sigma_delta(0.23) <= 1e-11, (integrator, split)
+
+
 def test_programme_per_turn_moments_every_turn_graph_and_plain():
     tr, p = both()
     z0, d0 = wl.gaussian_bunch(20_001, 0.23, 25)

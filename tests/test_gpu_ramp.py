@@ -108,6 +108,21 @@ def test_flat_ramp_without_tables_is_the_plain_map(integrator):
         assert_close(p, zg, dg, zp, dp, gate=1e-11)
 
 
+@pytest.mark.parametrize("turns", [1, 2, 10, 11, 31, 32, 33, 64, 65])
+def test_ramp_call_lengths_around_the_staging_block(turns):
+    """The fused kernel stages 32 sub-steps per block in a cp.async double buffer (Ruth4: 3 per
+    turn, so 10/11 turns straddle a block): lengths around the block size, merged and split."""
+    p0c, a, psi = wl.energy_ramp(turns, 26e9, 26e9 * (1 + 1e-5 * turns))
+    for integrator in INTEGRATORS:
+        tr, p = both(integrator, 0.5)
+        z0, d0 = wl.gaussian_bunch(777, 0.1, 47, ratio2=0.5)
+        zo, do = oracle.track_ramp(p, z0, d0, p0c, a, psi)
+        for split in (0, 1):
+            tr.set_option(lt.OPT_SPLIT_DRIFTS, split)
+            zg, dg = gpu_ramp(tr, z0, d0, p0c, a, psi)
+            assert_close(p, zg, dg, zo, do, gate=1e-11)
+
+
 def test_ramp_per_turn_moments_every_turn_graph_and_plain():
     tr, p = both()
     z0, d0 = wl.gaussian_bunch(20_001, 0.1, 44)
