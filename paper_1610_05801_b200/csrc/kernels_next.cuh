@@ -46,9 +46,9 @@ struct SliceAcc {
     int S, stride, rep_mask;
     __device__ __forceinline__ void init(const TurnExtras& X, unsigned long long turn,
                                          unsigned int* smem) {
-        sh = smem; S = X.n_slices; stride = S + 2; rep_mask = X.replicas - 1;
+        sh = smem; S = X.n_slices; stride = (S + 2) | 1; rep_mask = X.replicas - 1;   // odd stride: the copies of one slice sit in different banks
         z_lo = X.z_lo; z_hi = X.z_hi; inv = X.inv;
-        out = X.hist + turn * (unsigned long long)stride;
+        out = X.hist + turn * (unsigned long long)(S + 2);
         if (X.replicas > 0) {
             for (int i = threadIdx.x; i < X.replicas * stride; i += blockDim.x) sh[i] = 0u;
             __syncthreads();
@@ -62,7 +62,7 @@ struct SliceAcc {
     __device__ __forceinline__ void flush() {
         if (rep_mask < 0) return;
         __syncthreads();
-        for (int b = threadIdx.x; b < stride; b += blockDim.x) {
+        for (int b = threadIdx.x; b < S + 2; b += blockDim.x) {
             unsigned int c = 0u;
             for (int r = 0; r <= rep_mask; ++r) c += sh[r * stride + b];
             if (c) atomicAdd(out + b, (unsigned long long)c);

@@ -119,10 +119,14 @@ struct ExtraArgs {
     int n_slices;
 };
 
-// shared-memory copies of the histogram: as many as fit 32 KB per CTA, at most 8
+size_t slice_stride(int n_slices) { return ((size_t)n_slices + 2) | 1; }
+
+// shared-memory copies of the histogram
 int slice_replicas(int n_slices) {
-    const size_t one = ((size_t)n_slices + 2) * sizeof(unsigned int);
-    int r = 8;
+    // one copy per lane when they fit (no two lanes of a warp ever share a counter), halved until
+    // the copies fit 32 KB per CTA; the stride is made odd (see SliceAcc)
+    const size_t one = slice_stride(n_slices) * sizeof(unsigned int);
+    int r = 32;
     while (r > 0 && (size_t)r * one > 32 * 1024) r >>= 1;
     return r;
 }
@@ -149,7 +153,7 @@ template <int INTEG, int HARM>
 cudaError_t launch_extra_one(double* z, double* d, size_t n, int reverse, double* partials,
                              bool moments, bool vec_ok, int grid, const MapConsts<double>& c,
                              const TurnExtras& X, cudaStream_t st) {
-    const size_t smem = (size_t)X.replicas * ((size_t)X.n_slices + 2) * sizeof(unsigned int);
+    const size_t smem = (size_t)X.replicas * slice_stride(X.n_slices) * sizeof(unsigned int);
     if (vec_ok) {
         if (moments)
             per_turn_extra_kernel<INTEG, HARM, true, kPerTurnUnroll><<<grid, kPerTurnThreads, smem, st>>>(z, d, n, reverse, partials, c, X);
@@ -507,7 +511,7 @@ int lt_slice_histogram(lt_tracker* tr, const double* z_dev, size_t n, double z_l
     constexpr int kUnr = 4;                                   // 64 B in flight per thread
     size_t g = (n + 256 * 2 * kUnr - 1) / (256 * 2 * kUnr);
     g = std::max<size_t>(1, std::min<size_t>(g, (size_t)tr->sm_count * 8));
-    const size_t smem = (size_t)X.replicas * ((size_t)n_slices + 2) * sizeof(unsigned int);
+    const size_t smem = (size_t)X.replicas * slice_stride(n_slices) * sizeof(unsigned int);
     slice_histogram_kernel<kUnr><<<(unsigned)g, 256, smem, st>>>(z_dev, n, X);
     LT_CUDA(tr, cudaGetLastError());
     tr->launches++;
