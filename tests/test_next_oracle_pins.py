@@ -28,9 +28,9 @@ def small_bunch(n=200, seed=3, sigma_z=0.23):
 
 
 # ================================================================== f2: RF programme
-def programme_rows():
+def programme_rows(name="programme_values.txt"):
     rows, a, psi = [], None, None
-    for line in open(os.path.join(GOLD, "programme_values.txt")):
+    for line in open(os.path.join(GOLD, name)):
         if line.startswith("# volt_scale"):
             a = [float(x) for x in line.split("=")[1].split()]
         elif line.startswith("# phase_off"):
@@ -52,6 +52,22 @@ def test_programme_hand_iterated_values():
         z_ref, d_ref = float(z_ref), float(d_ref)
         assert abs(z[0] - z_ref) <= 1e-14 * max(abs(z_ref), 0.1), (name, r, z0, d0, t)
         assert abs(d[0] - d_ref) <= 1e-14 * max(abs(d_ref), 1e-3), (name, r, z0, d0, t)
+
+
+def test_programme_hand_iterated_values_with_synchronous_phase():
+    """The same programme at phi_s = 0.3 and -0.7, r = 0 and 0.25
+    (tests/golden/programme_phi_s_values.txt, mpmath only): pins the phi_s branch of
+    programme.inc -- sign of phi_s, sin(phi_s) subtracted unshifted by psi_t but scaled by a_t,
+    no phi_s in the 2h term (G3, G28)."""
+    rows, a, psi = programme_rows("programme_phi_s_values.txt")
+    assert len(rows) == 3 * 2 * 2 * 4 * 4
+    for name, phi, r, z0, d0, t, z_ref, d_ref in rows:
+        t = int(t)
+        p = oracle.make_params(wl.RING, name, float(r), phi_s=float(phi))
+        z, d = oracle.track_programme(p, [float(z0)], [float(d0)], a[:t], psi[:t])
+        z_ref, d_ref = float(z_ref), float(d_ref)
+        assert abs(z[0] - z_ref) <= 1e-14 * max(abs(z_ref), 0.1), (name, phi, r, z0, d0, t)
+        assert abs(d[0] - d_ref) <= 1e-14 * max(abs(d_ref), 1e-3), (name, phi, r, z0, d0, t)
 
 
 @pytest.mark.parametrize("integrator", INTEGRATORS)

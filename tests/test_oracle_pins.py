@@ -68,6 +68,49 @@ def test_hand_iterated_values():
         assert abs(d[0] - d_ref) <= tol * max(abs(d_ref), 1e-3), (name, r, z0, d0, t)
 
 
+def test_hand_iterated_values_with_synchronous_phase():
+    """Reading G3, F(z) = A[sin(phi_s + kappa z) - sin(phi_s) + r sin(2 kappa z)], iterated by
+    hand in 40 digits at phi_s = 0.3 and -0.7 (tests/golden/phi_s_values.txt, mpmath only).
+    The linear half-trace pin below sees only cos(phi_s): this one fails on a flipped sign of
+    phi_s, a missing - sin(phi_s), phi_s leaking into the 2h term, or any stand-in that merely
+    agrees to first order (e.g. cos(phi_s) sin(kappa z))."""
+    rows = [l.split() for l in open(os.path.join(GOLD, "phi_s_values.txt")) if l[0] != "#"]
+    assert len(rows) == 3 * 2 * 2 * 4 * 3
+    seen = set()
+    for name, phi, r, z0, d0, t, z_ref, d_ref in rows:
+        p = oracle.make_params(wl.RING, name, float(r), phi_s=float(phi))
+        z, d = oracle.track(p, [float(z0)], [float(d0)], int(t))
+        z_ref, d_ref = float(z_ref), float(d_ref)
+        tol = 1e-14 if int(t) <= 3 else 1e-11
+        assert abs(z[0] - z_ref) <= tol * max(abs(z_ref), 0.1), (name, phi, r, z0, d0, t)
+        assert abs(d[0] - d_ref) <= tol * max(abs(d_ref), 1e-3), (name, phi, r, z0, d0, t)
+        seen.add((name, phi, r))
+    assert len(seen) == 12
+
+
+def test_synchronous_phase_values_discriminate_the_plausible_mistakes():
+    """The golden values above are far (>= 1e-8) from what the wrong formulas give after one
+    turn, so the 1e-14 gate separates them: sign of phi_s, dropped sin(phi_s), first-order
+    stand-in.  Evaluated here in plain Python floats from the golden constants."""
+    g = golden_constants()
+    rows = [l.split() for l in open(os.path.join(GOLD, "phi_s_values.txt")) if l[0] != "#"]
+    for name, phi, r, z0, d0, t, z_ref, d_ref in rows:
+        if name != "euler_cromer" or t != "1":
+            continue
+        phi, r, z0, d0, d_ref = float(phi), float(r), float(z0), float(d0), float(d_ref)
+        kz = g["kappa"] * z0
+        right = d0 + g["A"] * (math.sin(phi + kz) - math.sin(phi) + r * math.sin(2 * kz))
+        assert abs(right - d_ref) <= 1e-15
+        wrong = (d0 + g["A"] * (math.sin(-phi + kz) - math.sin(-phi) + r * math.sin(2 * kz)),
+                 d0 + g["A"] * (math.sin(phi + kz) + r * math.sin(2 * kz)),
+                 d0 + g["A"] * (math.cos(phi) * math.sin(kz) + r * math.sin(2 * kz)),
+                 d0 + g["A"] * (math.sin(phi + kz) - math.sin(phi) + r * math.sin(2 * (kz + phi))))
+        if r == 0.0:
+            wrong = wrong[:3]             # no 2h term for phi_s to leak into
+        if z0 != 0.0:
+            assert all(abs(w - d_ref) >= 1e-8 for w in wrong), (phi, r, z0)
+
+
 def test_first_hand_value_by_pocket_calculator():
     """(z, delta) = (0.1, 0): the first half drift leaves z, the kick is A sin(kappa*0.1),
     the second half drift subtracts d times it."""
