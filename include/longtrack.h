@@ -313,6 +313,18 @@ int lt_track_transverse_per_turn(lt_tracker *tr, double *x_dev, double *xp_dev, 
  * per chain) and returns achieved FP64 lane-instructions per second in *rate. Synchronises. */
 int lt_probe_fp64(int blocks, int threads, int chains, long long iters, double *rate_host,
                   double *ms_host);
+/* What the FP64 pipe of the device at hand issues, counted with clock64 (so independent of the
+ * clock): `threads` (multiple of 32, <= 1024) threads in each of `blocks` CTAs (one CTA per SM:
+ * pass the SM count) run `chains` (1, 2, 4) independent dependent chains of 8 * iters steps of
+ *   kind 0  DFMA with three register operands      kind 1  DFMA, two registers + a uniform operand
+ *   kind 2  DADD                                   kind 3  DMUL
+ *   kind 10 / 11 / 12  the 13-instruction leap-frog turn of the fused kernel
+ *                      with the sign flip on the polynomial / on the argument / left out.
+ * *instr_per_cycle_host = FP64 warp-instructions per cycle and SM sub-partition (the pipe's
+ * nominal peak is 0.5: 16 lanes per sub-partition); *sm_clock_mhz_host (may be NULL) = SM clock
+ * during the probe, from clock64 against the nanosecond global timer.  Synchronises. */
+int lt_probe_pipe(int kind, int blocks, int threads, int chains, long long iters,
+                  double *instr_per_cycle_host, double *sm_clock_mhz_host);
 
 #ifdef __cplusplus
 }

@@ -67,11 +67,12 @@ template <> struct Real<double> {
     static __device__ __forceinline__ double sub(double a, double b) { return __dsub_rn(a, b); }
     static __device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
     // f with the sign bit flipped when the integer held in the low mantissa bits of t is odd.
-    // hi + (lo << 31) mod 2^32 == hi ^ ((lo & 1) << 31): ONE IMAD instead of shift + xor (every
-    // non-FP64 instruction in the turn loop costs about two issue cycles, profiles/r1_fused_sweep.md).
+    // hi + (lo << 31) mod 2^32 == hi ^ ((lo & 1) << 31): ONE IMAD instead of shift + xor, in
+    // unsigned arithmetic (defined on overflow).  Next to a saturated FP64 pipe the IMAD costs
+    // 2.6 points of the pipe, a shift + LOP3 pair 12 (profiles/r2_fp64_pipe_probe.md).
     static __device__ __forceinline__ double flip(double f, double t) {
-        int hi = __double2hiint(f) + __double2loint(t) * (int)0x80000000;
-        return __hiloint2double(hi, __double2loint(f));
+        const unsigned int hi = (unsigned int)__double2hiint(f) + ((unsigned int)__double2loint(t) << 31);
+        return __hiloint2double((int)hi, __double2loint(f));
     }
     static __device__ __forceinline__ double flip_by(double x, double t) { return flip(x, t); }
 };
@@ -85,7 +86,7 @@ template <> struct Real<float> {
     static __device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
     static __device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
     static __device__ __forceinline__ float flip(float f, float t) {
-        return __int_as_float(__float_as_int(f) + __float_as_int(t) * (int)0x80000000);
+        return __uint_as_float(__float_as_uint(f) + (__float_as_uint(t) << 31));
     }
     static __device__ __forceinline__ float flip_by(float x, float t) { return flip(x, t); }
 };
@@ -123,35 +124,36 @@ __device__ __forceinline__ T horner(const T (&c)[N], T s) {
 //     a * A [ sin(phi_s + pi (v + p)) - sin(phi_s) + r sin(2 pi (v + p)) ],
 // a = voltage scale, p = phase offset in half periods.  PROG = 1: add p here (fast path, the
 // state is v); PROG = 2: the caller already folded p into v (exact path: v = fma(z, kappa/pi, p)).
-// PROG = 3 / 4 (energy ramp, G32): as 1 / 2, but `a` is the ABSOLUTE kick amplitude
-// tau a_t A(p_b) of the sub-step, so the unscaled polynomial sin(pi f)/f is used.
+// The scale multiplies f, not q: f*a is ready three instructions after the reduction and runs
+// beside the Horner chain, so the dependent chain of a turn is one FP64 instruction shorter than
+// with q*a behind the polynomial (same 15 instructions; a = 1 still returns the plain map's bits).
 template <typename T, int HARM, bool FQ = false, int PROG = 0>
 __device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage, T a = T(1),
                                   T p = T(0)) {
     typedef Real<T> R;
     constexpr int NS = R::NS, NC = R::NC;
-    static_assert(PROG < 3 || HARM != 0, "the energy ramp has no generic phi_s path");
-    const T (&sin_coef)[kMaxSin] = PROG >= 3 ? P.sin1 : P.sinA[stage];
-    if (PROG == 1 || PROG == 3) v = R::add(v, p);
+    static_assert(PROG >= 0 && PROG <= 2, "the energy ramp has its own kick (kernels_ramp.cuh)");
+    const T (&sin_coef)[kMaxSin] = P.sinA[stage];
+    if (PROG == 1) v = R::add(v, p);
     if (HARM == 1) {
         T t;
         T f = reduce_half_periods(v, &t);
         T s = R::mul(f, f);
+        T fa = PROG ? R::mul(f, a) : f;
         T q = horner<T, NS>(sin_coef, s);
-        if (PROG) q = R::mul(q, a);
-        if (FQ) return R::fma(f, R::flip(q, t), delta);
-        return R::fma(R::flip(f, t), q, delta);
+        if (FQ) return R::fma(fa, R::flip(q, t), delta);
+        return R::fma(R::flip(fa, t), q, delta);
     } else if (HARM == 2) {
         T t;
         T f = reduce_half_periods(v, &t);
         T s = R::mul(f, f);
+        T fa = PROG ? R::mul(f, a) : f;
         T q = horner<T, NS>(sin_coef, s);         // tau A sin(pi f)/f
         T c = horner<T, NC>(P.cos1, s);           // cos(pi f)
-        if (PROG) q = R::mul(q, a);
         // sin and cos both change sign with the parity of n: flip f, and flip 2r for the cos
         T m = R::fma(R::flip_by(P.two_r, t), c, T(1));
-        if (FQ) return R::fma(f, R::flip(R::mul(q, m), t), delta);
-        return R::fma(R::flip(f, t), R::mul(q, m), delta);
+        if (FQ) return R::fma(fa, R::flip(R::mul(q, m), t), delta);
+        return R::fma(R::flip(fa, t), R::mul(q, m), delta);
     } else {
         T t1, t2;
         T f1 = reduce_half_periods(R::add(v, P.phi_off), &t1);
@@ -198,21 +200,26 @@ __device__ __forceinline__ void turn_exact(T& z, T& delta, const MapConsts<T>& P
 // One turn on the FAST path, state = phase v, WITHOUT its leading drift and with the trailing
 // drift given by the caller (merged with the next turn's leading drift, or the plain trailing
 // one at the end of a call).
+// PROG: the state is u = v + p_t, the phase INCLUDING this turn's RF phase offset; dp = p_(t+1) - p_t
+// is added to u beside the sine chain and the trailing drift is an FMA onto that sum, so the
+// offset costs one FP64 instruction and none on the dependent chain.
 template <typename T, int INTEG, int HARM, bool FQ = false, bool PROG = false>
 __device__ __forceinline__ void turn_fast(T& v, T& delta, const MapConsts<T>& P, T trailing,
-                                          T a = T(1), T p = T(0)) {
+                                          T a = T(1), T dp = T(0)) {
     typedef Real<T> R;
-    constexpr int PK = PROG ? 1 : 0;
+    constexpr int PK = PROG ? 2 : 0;
     if (INTEG == kRuth4) {
-        delta = kick<T, HARM, FQ, PK>(v, delta, P, 0, a, p);
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 0, a);
         v = R::fma(-P.drift_mid, delta, v);
-        delta = kick<T, HARM, FQ, PK>(v, delta, P, 1, a, p);
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 1, a);
         v = R::fma(-P.drift_mid, delta, v);
-        delta = kick<T, HARM, FQ, PK>(v, delta, P, 2, a, p);
-        v = R::fma(-trailing, delta, v);
+        const T w = PROG ? R::add(v, dp) : v;
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 2, a);
+        v = R::fma(-trailing, delta, w);
     } else {
-        delta = kick<T, HARM, FQ, PK>(v, delta, P, 0, a, p);
-        v = R::fma(-trailing, delta, v);
+        const T w = PROG ? R::add(v, dp) : v;
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 0, a);
+        v = R::fma(-trailing, delta, w);
     }
 }
 
@@ -221,8 +228,10 @@ __device__ __forceinline__ void turn_fast(T& v, T& delta, const MapConsts<T>& P,
 // trailing drift and converts back, in between consecutive half drifts are merged.  Between
 // chunks of one call the z array therefore holds v mid-drift, which makes the result of a
 // call independent of how its turns are chunked.  SPLIT: exact path, state is z.
-// PROG: prog[k] = (a, p) of the k-th turn of this call to advance (voltage scale, phase offset
-// in half periods; one uniform 16-byte load per turn and warp).
+// PROG: prog[k] = (a, p) of the k-th turn of this call to advance on the exact path (voltage
+// scale, phase offset in half periods); on the fast path prog[k] = (a, p_(k+1) - p_k) -- the
+// difference to the NEXT turn's offset, minus the last offset at the end of the API call -- and
+// prog[-1].y = the absolute offset of turn 0 of the launch (used by `first` only).
 template <typename T, int INTEG, int HARM, bool SPLIT, int ILP, bool FQ, bool PROG = false>
 __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int turns, int first,
                                         int last, const MapConsts<T>& P,
@@ -237,10 +246,12 @@ __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int 
         // of the FP64 peak; profiles/r1_next_rows_ncu.md).
         const unsigned int lane = threadIdx.x & 31u;
         if (!SPLIT && first) {
+            const T p0 = (T)__ldg(prog - 1).y;
 #pragma unroll
             for (int j = 0; j < ILP; ++j) {
                 x[j] = R::mul(x[j], P.to_phase);
                 if (INTEG != kEulerCromer) x[j] = R::fma(-P.drift_lead, dl[j], x[j]);
+                x[j] = R::add(x[j], p0);
             }
         }
         // the fast path peels the last turn (its trailing drift differs at the end of a call)
@@ -389,6 +400,45 @@ __global__ void fused_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_
 // The arithmetic per particle is identical to fused_kernel, so results are bit-identical to it
 // and independent of item_turns and of the scheduling order.
 // ------------------------------------------------------------------------------------------
+// Work-item schedule of the persistent kernels: a launch of `turns` turns is cut into chunks, the
+// same for every group of particles.  Plain: ceil(turns / item) chunks of `item` turns.  Tapered
+// (dynamic scheduling): full items first, then the last item..2*item turns are halved again and
+// again down to kMinTaper turns, so that the warps which find the ticket queue empty wait for a
+// short item, not a long one (an untapered tail cost 1.7 % at 10^5 particles,
+// profiles/r2_item_sweep.md).  Chunk boundaries never change the arithmetic (G16).
+constexpr unsigned int kMinTaper = 64;
+struct ItemSchedule {
+    unsigned int turns, item, nfull, nchunks;
+    __host__ __device__ void init(unsigned int turns_, unsigned int item_, int taper) {
+        turns = turns_; item = item_ < 1u ? 1u : item_;
+        if (!taper) {
+            nfull = turns / item;
+            nchunks = (turns + item - 1) / item;
+            return;
+        }
+        const unsigned int q = turns / item;
+        nfull = q > 0 ? q - 1 : 0;
+        unsigned int r = turns - nfull * item, k = 0;
+        while (r > 0) { const unsigned int len = r <= kMinTaper ? r : (r + 1) / 2; r -= len; ++k; }
+        nchunks = nfull + k;
+    }
+    // first turn and length of chunk c
+    __host__ __device__ void span(unsigned int c, int taper, unsigned int* start, unsigned int* len) const {
+        if (!taper || c < nfull) {
+            *start = c * item;
+            *len = (turns - *start < item) ? turns - *start : item;
+            return;
+        }
+        unsigned int s0 = nfull * item, r = turns - s0, l = 0;
+        for (unsigned int k = nfull;; ++k) {
+            l = r <= kMinTaper ? r : (r + 1) / 2;
+            if (k == c) break;
+            s0 += l; r -= l;
+        }
+        *start = s0; *len = l;
+    }
+};
+
 __device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
     unsigned int v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -399,17 +449,25 @@ __device__ __forceinline__ void st_release_u32(unsigned int* p, unsigned int v) 
 }
 
 // PROG: prog[k] = (a, p) of the k-th turn of THIS launch (RF programme, f2).
-template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ, bool PROG = false>
-__global__ void __launch_bounds__(1024, 1)
+// ILP: particles per lane.  A work item is (chunk) x (group of 32*ILP particles); particle j of a
+// lane is element g*32*ILP + 32*j + lane (coalesced).  Two independent chains per warp issue
+// back to back without a warp switch: the turn loop measures 91.5 % of the FP64 peak at 4 chains
+// per sub-partition as 2 warps x 2 chains against 87.5 % as 4 warps x 1 chain
+// (profiles/r2_fp64_pipe_probe.md).  The arithmetic per particle does not depend on ILP.
+template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ, bool PROG = false, int ILP = 1>
+__global__ void __launch_bounds__(ILP == 1 ? 1024 : 512, 1)
 fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, unsigned int turns,
                         unsigned int item_turns, int first_launch, int last_launch, int dynamic,
                         unsigned long long* __restrict__ ticket, unsigned int* __restrict__ done,
                         const __grid_constant__ MapConsts<T> P,
                         const double2* __restrict__ prog = nullptr) {
     extern __shared__ __align__(16) unsigned char residency_cap[];   // sized to cap CTAs per SM; PROG: 512 B per warp of staged programme entries
+    constexpr unsigned int G = 32u * ILP;
     const unsigned int lane = threadIdx.x & 31u;
-    const unsigned long long groups = (n + 31) / 32;
-    const unsigned int nchunks = (turns + item_turns - 1) / item_turns;
+    const unsigned long long groups = (n + G - 1) / G;
+    ItemSchedule sched;
+    sched.init(turns, item_turns, dynamic);
+    const unsigned int nchunks = sched.nchunks;
     const unsigned long long total = groups * nchunks;
     // static mode (few groups): slot s of the grid owns groups s, s + S, ... for all turns;
     // slots are numbered SM-first so that groups spread evenly over SMs and sub-partitions
@@ -429,17 +487,26 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
         if (c > 0) {
             while (ld_acquire_u32(done + g) < c) __nanosleep(64);
         }
-        const size_t i = (size_t)g * 32 + lane;
-        T x[1], dl[1];
-        x[0] = (i < n) ? __ldcg(z_arr + i) : T(0);      // L2 only: another SM may have written it
-        dl[0] = (i < n) ? __ldcg(d_arr + i) : T(0);
+        const size_t i0 = (size_t)g * G + lane;
+        T x[ILP], dl[ILP];
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            const size_t i = i0 + 32u * j;
+            x[j] = (i < n) ? __ldcg(z_arr + i) : T(0);   // L2 only: another SM may have written it
+            dl[j] = (i < n) ? __ldcg(d_arr + i) : T(0);
+        }
         const int first = first_launch && c == 0;
         const int last = last_launch && c == nchunks - 1;
-        const unsigned int nt = (c == nchunks - 1) ? turns - c * item_turns : item_turns;
-        advance<T, INTEG, HARM, SPLIT, 1, FQ, PROG>(
-            x, dl, nt, first, last, P, PROG ? prog + (size_t)c * item_turns : nullptr,
+        unsigned int t_start, nt;
+        sched.span(c, dynamic, &t_start, &nt);
+        advance<T, INTEG, HARM, SPLIT, ILP, FQ, PROG>(
+            x, dl, nt, first, last, P, PROG ? prog + t_start : nullptr,
             PROG ? reinterpret_cast<double2*>(residency_cap) + (threadIdx.x & ~31u) : nullptr);
-        if (i < n) { __stcg(z_arr + i, x[0]); __stcg(d_arr + i, dl[0]); }
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            const size_t i = i0 + 32u * j;
+            if (i < n) { __stcg(z_arr + i, x[j]); __stcg(d_arr + i, dl[j]); }
+        }
         if (nchunks > 1) {
             __threadfence();
             __syncwarp();

@@ -213,12 +213,26 @@ static __global__ void slice_histogram_kernel(const double* __restrict__ z_arr, 
     sl.flush();
 }
 
-// Programme tables for the fused kernel: (a_t, psi_t / pi) packed as double2.
+// Programme table of one fused launch, double2 per turn behind a one-entry header:
+//   exact path:  out[1 + i] = (a_T, p_T),          p_T = psi_T / pi,  T = t_first + i
+//   fast path:   out[1 + i] = (a_T, p_(T+1) - p_T), with p_(call_turns) := 0 (the state leaves the
+//                call as the plain phase);  out[0].y = p_(t_first) for the launch's first turn.
 static __global__ void programme_pack_kernel(const double* __restrict__ volt_scale,
-                                      const double* __restrict__ phase_off, unsigned int count,
-                                      double inv_pi, double2* __restrict__ out) {
+                                      const double* __restrict__ phase_off,
+                                      unsigned long long t_first, unsigned int count,
+                                      unsigned long long call_turns, double inv_pi, int fast,
+                                      double2* __restrict__ out) {
     const unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < count) out[i] = make_double2(volt_scale[i], __dmul_rn(phase_off[i], inv_pi));
+    if (i >= count) return;
+    const unsigned long long T = t_first + i;
+    const double p = __dmul_rn(phase_off[T], inv_pi);
+    if (i == 0) out[0] = make_double2(0.0, p);
+    if (fast) {
+        const double pn = (T + 1 < call_turns) ? __dmul_rn(phase_off[T + 1], inv_pi) : 0.0;
+        out[1 + i] = make_double2(volt_scale[T], __dsub_rn(pn, p));
+    } else {
+        out[1 + i] = make_double2(volt_scale[T], p);
+    }
 }
 
 // ------------------------------------------------------------------------------------------
@@ -310,7 +324,9 @@ transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp
     constexpr unsigned int G = 32u * ILP;
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned long long groups = (n + G - 1) / G;
-    const unsigned int nchunks = (turns + item_turns - 1) / item_turns;
+    ItemSchedule sched;
+    sched.init(turns, item_turns, dynamic);
+    const unsigned int nchunks = sched.nchunks;
     const unsigned long long total = groups * nchunks;
     const unsigned long long slots = (unsigned long long)gridDim.x * (blockDim.x >> 5);
     unsigned long long next = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
@@ -331,7 +347,8 @@ transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp
         const size_t i0 = (size_t)g * G + lane;
         const int first = first_launch && c == 0;
         const int last = last_launch && c == nchunks - 1;
-        const unsigned int nt = (c == nchunks - 1) ? turns - c * item_turns : item_turns;
+        unsigned int t_start, nt;
+        sched.span(c, dynamic, &t_start, &nt);
         double u[ILP][4], v[ILP], dl[ILP];
 #pragma unroll
         for (int j = 0; j < ILP; ++j) {

@@ -11,6 +11,10 @@
 // with amp = tau a_t A(p_b), g = p_b/p_a, c = -(p_a - p_b)/p_a, db = tau d(p_b), da = tau d(p_a)
 // (Euler-Cromer: db = 0, da = 2 d(p_a)).  ramp_pack_kernel turns the caller's tables into one
 // 48-byte entry per sub-step; the tracking kernels are then generic in the integrator.
+// The kick line is evaluated as  delta = (g amp) [..] + (g delta + c):  the product g*amp comes
+// from the pack kernel, f*(g amp) and g*delta + c run BESIDE the Horner chain, and the last FMA
+// of the sine is the whole update -- the dependent chain of a sub-step is 14 FP64 instructions
+// of its 17 (it was 16 with q*amp, the kick FMA and the damping FMA in a row).
 #pragma once
 
 #include "kernels.cuh"
@@ -18,12 +22,16 @@
 namespace lt {
 
 // One sub-step, 48 bytes = three double2.
-//   exact layout (split drifts, per-turn kernel):  d0 = db, d1 = da                (metres)
-//   fast layout (merged drifts, state = phase v):  d0 = (da + db of the NEXT sub-step) kappa/pi,
-//                                                  d1 = db kappa/pi (used by the call's first sub-step)
+//   exact layout (split drifts, per-turn kernel):  p = psi/pi;  d0 = db, d1 = da      (metres)
+//   fast layout (merged drifts, state = phase u = v + p INCLUDING the sub-step's RF phase offset):
+//       p  = (psi of the NEXT sub-step - psi of this one)/pi, minus the last psi/pi at the end of
+//            the API call, so that the offset is one DADD beside the sine chain and the state
+//            leaves the call as the plain phase;
+//       d0 = (da + db of the NEXT sub-step) kappa/pi,  d1 = db kappa/pi (the call's first sub-step)
+//   The fast table starts with a header entry whose p is the absolute psi/pi of its first sub-step.
 struct RampEntry {
-    double amp, p;      // kick amplitude; psi/pi (RF phase offset in half periods)
-    double g, c;        // delta <- g * delta + c after the kick
+    double ga, p;       // g * kick amplitude; RF phase offset in half periods (see the layouts)
+    double g, c;        // delta <- g * (delta + kick) + c
     double d0, d1;
 };
 
@@ -56,6 +64,7 @@ static __global__ void ramp_pack_kernel(const double* __restrict__ p0c, const do
     const double pb = p0c[T], pa = p0c[T + 1];
     const double av = volt ? volt[T] : 1.0;
     const double psi = phase ? phase[T] : 0.0;
+    const double psi_next = (phase && T + 1 < call_turns) ? phase[T + 1] : 0.0;
     const int nsub = integ == kRuth4 ? 3 : 1;
     double ps[4], tau[3];
     ps[0] = pb;
@@ -72,11 +81,18 @@ static __global__ void ramp_pack_kernel(const double* __restrict__ p0c, const do
     double A[4], d[4];
     for (int k = 0; k <= nsub; ++k) ramp_ring_at(R, ps[k], &A[k], &d[k]);
     const double tau_first = integ == kEulerCromer ? 0.0 : tau[0];
+    const double p_here = __dmul_rn(psi, R.inv_pi);
+    RampEntry* dst = out + (fast ? 1 : 0);                 // fast layout: behind the header entry
+    if (fast && i == 0) {
+        RampEntry h;
+        h.ga = 0.0; h.p = p_here; h.g = 1.0; h.c = 0.0; h.d0 = 0.0; h.d1 = 0.0;
+        out[0] = h;
+    }
     for (int k = 0; k < nsub; ++k) {
         RampEntry e;
-        e.amp = tau[k] * A[k] * av;
-        e.p = psi * R.inv_pi;
         e.g = ps[k] / ps[k + 1];
+        e.ga = e.g * (tau[k] * A[k] * av);
+        e.p = p_here;
         e.c = -(ps[k + 1] - ps[k]) / ps[k + 1];
         double db = tau[k] * d[k], da = tau[k] * d[k + 1];
         if (integ == kEulerCromer) { db = 0.0; da = 2.0 * d[1]; }
@@ -86,11 +102,13 @@ static __global__ void ramp_pack_kernel(const double* __restrict__ p0c, const do
             else db_next = (T + 1 == call_turns) ? 0.0 : tau_first * d[nsub];
             e.d0 = (da + db_next) * R.to_phase;
             e.d1 = db * R.to_phase;
+            // every sub-step of a turn sees the same psi: the offset changes behind the last one
+            e.p = (k + 1 < nsub) ? 0.0 : __dsub_rn(__dmul_rn(psi_next, R.inv_pi), p_here);
         } else {
             e.d0 = db;
             e.d1 = da;
         }
-        out[(size_t)i * nsub + k] = e;
+        dst[(size_t)i * nsub + k] = e;
     }
 }
 
@@ -98,27 +116,46 @@ static __global__ void ramp_advance_cursor_kernel(unsigned long long* cursor, un
     *cursor += by;
 }
 
+// delta <- g (delta + amp F) + c  for the phase v (half periods, psi already added):
+//     fma(+-f ga, sin(pi f)/f [(1 + 2 r cos(pi f))], fma(g, delta, c)),   ga = g amp
+template <int HARM>
+__device__ __forceinline__ double ramp_kick(double v, double dl, const MapConsts<double>& P,
+                                            double ga, double g, double c) {
+    typedef Real<double> R;
+    double t;
+    const double f = reduce_half_periods(v, &t);
+    const double s = __dmul_rn(f, f);
+    const double fa = __dmul_rn(f, ga);
+    const double base = __fma_rn(g, dl, c);
+    double q = horner<double, R::NS>(P.sin1, s);
+    if (HARM == 2) {
+        const double cc = horner<double, R::NC>(P.cos1, s);
+        q = __dmul_rn(q, __fma_rn(R::flip_by(P.two_r, t), cc, 1.0));
+    }
+    return __fma_rn(R::flip(fa, t), q, base);
+}
+
 // exact sub-step: state z, every drift its own FMA (bit-identical between the fused split-drift
 // kernel, the per-turn kernel and any chunking)
 template <int HARM>
 __device__ __forceinline__ void ramp_substep_exact(double& z, double& dl, const MapConsts<double>& P,
-                                                   double amp, double p, double g, double c,
+                                                   double ga, double p, double g, double c,
                                                    double db, double da) {
     z = __fma_rn(-db, dl, z);
-    dl = kick<double, HARM, false, 4>(__fma_rn(z, P.to_phase, p), dl, P, 0, amp);
-    dl = __fma_rn(g, dl, c);
+    dl = ramp_kick<HARM>(__fma_rn(z, P.to_phase, p), dl, P, ga, g, c);
     z = __fma_rn(-da, dl, z);
 }
 
-// fast sub-step: state v (phase in half periods), trailing drift merged with the next leading one.
-// 17 FP64 instructions (single harmonic): v + p, 3 reduction, f^2, 7 Horner, q * amp, kick FMA,
-// damping FMA, drift FMA.
+// fast sub-step: state u = v + p (phase in half periods including the RF phase offset), trailing
+// drift merged with the next leading one.  16 FP64 instructions (single harmonic): 3 reduction,
+// f^2, f * ga, g * delta + c, u + dp, 7 Horner, the kick FMA, the drift FMA; 13 of them on the
+// dependent chain (reduction, f^2, Horner, kick, drift).
 template <int HARM>
-__device__ __forceinline__ void ramp_substep_fast(double& v, double& dl, const MapConsts<double>& P,
-                                                  double amp, double p, double g, double c, double dm) {
-    dl = kick<double, HARM, true, 3>(v, dl, P, 0, amp, p);
-    dl = __fma_rn(g, dl, c);
-    v = __fma_rn(-dm, dl, v);
+__device__ __forceinline__ void ramp_substep_fast(double& u, double& dl, const MapConsts<double>& P,
+                                                  double ga, double dp, double g, double c, double dm) {
+    const double w = __dadd_rn(u, dp);
+    dl = ramp_kick<HARM>(u, dl, P, ga, g, c);
+    u = __fma_rn(-dm, dl, w);
 }
 
 __device__ __forceinline__ void cp_async_16(void* smem_dst, const void* gmem_src) {
@@ -128,14 +165,14 @@ __device__ __forceinline__ void cp_async_16(void* smem_dst, const void* gmem_src
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 
-// `nsteps` sub-steps of one particle; tab = the item's first entry as double2[3 * nsteps]; stage =
-// the warp's private double buffer in shared memory (2 x 32 entries = 3072 B).  While the warp
-// works through one block of 32 entries, the next block arrives by cp.async (no registers held,
-// no L2 latency on the dependent FP64 chain; a per-sub-step global load stalled the RF-programme
-// kernel once per 128-byte line, profiles/r1_next_rows_ncu.md).
-template <int HARM, bool SPLIT>
-__device__ __forceinline__ void ramp_advance(double& x, double& dl, unsigned int nsteps, int first,
-                                             int last, const MapConsts<double>& P,
+// `nsteps` sub-steps of the ILP particles of a lane; tab = the item's first entry as
+// double2[3 * nsteps]; stage = the warp's private double buffer in shared memory (2 x 32 entries =
+// 3072 B).  While the warp works through one block of 32 entries, the next block arrives by
+// cp.async (no registers held, no L2 latency on the dependent FP64 chain; a per-sub-step global
+// load stalled the RF-programme kernel once per 128-byte line, profiles/r1_next_rows_ncu.md).
+template <int HARM, bool SPLIT, int ILP>
+__device__ __forceinline__ void ramp_advance(double (&x)[ILP], double (&dl)[ILP], unsigned int nsteps,
+                                             int first, int last, const MapConsts<double>& P,
                                              const double2* __restrict__ tab,
                                              double2* __restrict__ stage) {
     const unsigned int lane = threadIdx.x & 31u;
@@ -150,9 +187,13 @@ __device__ __forceinline__ void ramp_advance(double& x, double& dl, unsigned int
     };
     fetch(0, 0);
     if (!SPLIT && first) {
-        const double lead = __ldg(tab + 2).y;
-        x = __dmul_rn(x, P.to_phase);
-        x = __fma_rn(-lead, dl, x);
+        const double lead = __ldg(tab + 2).y, p0 = __ldg(tab - 3).y;   // header entry: absolute offset
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            x[j] = __dmul_rn(x[j], P.to_phase);
+            x[j] = __fma_rn(-lead, dl[j], x[j]);
+            x[j] = __dadd_rn(x[j], p0);
+        }
     }
     unsigned int buf = 0;
     for (unsigned int t0 = 0; t0 < nsteps; t0 += 32, buf ^= 1u) {
@@ -161,30 +202,40 @@ __device__ __forceinline__ void ramp_advance(double& x, double& dl, unsigned int
         __syncwarp();
         const double2* __restrict__ cur = stage + 96u * buf;
         const unsigned int m = min(32u, nsteps - t0);
-#pragma unroll 8
+        constexpr int kUnrollR = ILP > 1 ? 4 : 8;
+#pragma unroll kUnrollR
         for (unsigned int k = 0; k < m; ++k) {
             const double2 e0 = cur[3 * k], e1 = cur[3 * k + 1], e2 = cur[3 * k + 2];
-            if (SPLIT) ramp_substep_exact<HARM>(x, dl, P, e0.x, e0.y, e1.x, e1.y, e2.x, e2.y);
-            else ramp_substep_fast<HARM>(x, dl, P, e0.x, e0.y, e1.x, e1.y, e2.x);
+#pragma unroll
+            for (int j = 0; j < ILP; ++j) {
+                if (SPLIT) ramp_substep_exact<HARM>(x[j], dl[j], P, e0.x, e0.y, e1.x, e1.y, e2.x, e2.y);
+                else ramp_substep_fast<HARM>(x[j], dl[j], P, e0.x, e0.y, e1.x, e1.y, e2.x);
+            }
         }
         __syncwarp();                        // all lanes are done with `buf` before it is refilled
     }
-    if (!SPLIT && last) x = __dmul_rn(x, P.from_phase);
+    if (!SPLIT && last) {
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) x[j] = __dmul_rn(x[j], P.from_phase);
+    }
 }
 
 // Fused multi-turn kernel with the ramp: the persistent ticketed work queue of
 // fused_persistent_kernel (kernels.cuh), work item = (chunk of item_steps sub-steps) x (32 particles).
-template <int HARM, bool SPLIT>
-__global__ void __launch_bounds__(1024, 1)
+template <int HARM, bool SPLIT, int ILP>
+__global__ void __launch_bounds__(ILP == 1 ? 1024 : 512, 1)
 ramp_persistent_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, size_t n,
                        unsigned int nsteps, unsigned int item_steps, int first_launch, int last_launch,
                        int dynamic, unsigned long long* __restrict__ ticket,
                        unsigned int* __restrict__ done, const __grid_constant__ MapConsts<double> P,
                        const double2* __restrict__ table) {
     extern __shared__ __align__(16) unsigned char ramp_smem[];   // 3072 B per warp + residency cap
+    constexpr unsigned int G = 32u * ILP;
     const unsigned int lane = threadIdx.x & 31u;
-    const unsigned long long groups = (n + 31) / 32;
-    const unsigned int nchunks = (nsteps + item_steps - 1) / item_steps;
+    const unsigned long long groups = (n + G - 1) / G;
+    ItemSchedule sched;
+    sched.init(nsteps, item_steps, dynamic);
+    const unsigned int nchunks = sched.nchunks;
     const unsigned long long total = groups * nchunks;
     const unsigned long long slots = (unsigned long long)gridDim.x * (blockDim.x >> 5);
     unsigned long long next = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
@@ -203,14 +254,24 @@ ramp_persistent_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, s
         if (c > 0) {
             while (ld_acquire_u32(done + g) < c) __nanosleep(64);
         }
-        const size_t i = (size_t)g * 32 + lane;
-        double x = (i < n) ? __ldcg(z_arr + i) : 0.0;
-        double dl = (i < n) ? __ldcg(d_arr + i) : 0.0;
+        const size_t i0 = (size_t)g * G + lane;
+        double x[ILP], dl[ILP];
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            const size_t i = i0 + 32u * j;
+            x[j] = (i < n) ? __ldcg(z_arr + i) : 0.0;
+            dl[j] = (i < n) ? __ldcg(d_arr + i) : 0.0;
+        }
         const int first = first_launch && c == 0;
         const int last = last_launch && c == nchunks - 1;
-        const unsigned int ns = (c == nchunks - 1) ? nsteps - c * item_steps : item_steps;
-        ramp_advance<HARM, SPLIT>(x, dl, ns, first, last, P, table + 3 * (size_t)c * item_steps, stage);
-        if (i < n) { __stcg(z_arr + i, x); __stcg(d_arr + i, dl); }
+        unsigned int s_start, ns;
+        sched.span(c, dynamic, &s_start, &ns);
+        ramp_advance<HARM, SPLIT, ILP>(x, dl, ns, first, last, P, table + 3 * (size_t)s_start, stage);
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            const size_t i = i0 + 32u * j;
+            if (i < n) { __stcg(z_arr + i, x[j]); __stcg(d_arr + i, dl[j]); }
+        }
         if (nchunks > 1) {
             __threadfence();
             __syncwarp();
@@ -234,13 +295,13 @@ __global__ void ramp_per_turn_kernel(double* __restrict__ z_arr, double* __restr
 #pragma unroll
         for (int s = 0; s < NSUB; ++s) {
             const double2 a = __ldg(src + 3 * s), b = __ldg(src + 3 * s + 1), c = __ldg(src + 3 * s + 2);
-            e[s].amp = a.x; e[s].p = a.y; e[s].g = b.x; e[s].c = b.y; e[s].d0 = c.x; e[s].d1 = c.y;
+            e[s].ga = a.x; e[s].p = a.y; e[s].g = b.x; e[s].c = b.y; e[s].d0 = c.x; e[s].d1 = c.y;
         }
     }
     auto turn = [&](double& z, double& dl) {
 #pragma unroll
         for (int s = 0; s < NSUB; ++s)
-            ramp_substep_exact<HARM>(z, dl, P, e[s].amp, e[s].p, e[s].g, e[s].c, e[s].d0, e[s].d1);
+            ramp_substep_exact<HARM>(z, dl, P, e[s].ga, e[s].p, e[s].g, e[s].c, e[s].d0, e[s].d1);
     };
     Sums acc;
     acc.zero();

@@ -10,6 +10,7 @@
 #include <new>
 
 #include "sinpi_coeffs.h"
+#include "kernels_probe.cuh"
 
 using namespace lt;
 using namespace lt_host;
@@ -210,61 +211,73 @@ cudaError_t launch_fused_integ(int harm, bool split, T* z, T* d, size_t n, unsig
 // pinned by a dummy dynamic shared-memory request so that the CTA scheduler cannot stack two on
 // one SM and leave another empty.
 // ------------------------------------------------------------------------------------------
-// FP64 warp-instructions per cycle per sub-partition of the turn loop at W resident warps
-// (measured with clock64 on B200, profiles/r1_fused_sweep.md): sign flip on f / on q
-double loop_rate(int w, bool fq) {
-    static const double on_f[] = {0, .1229, .2424, .3546, .4367, .4367, .4399, .4418, .4428};
-    static const double on_q[] = {0, .1200, .2380, .3480, .4259, .4414, .4554, .4590, .4613};
+// FP64 warp-instructions per cycle per sub-partition of the turn loop (peak 0.5) at W resident
+// warps carrying ILP independent particles per lane, sign flip on f / on q: measured with clock64
+// on B200 (profiles/r2_fp64_pipe_probe.md).  Two chains per warp saturate the pipe with half the
+// warps, and with them the flip on f wins; with one chain per warp the flip on q wins from W = 5.
+double loop_rate(int ilp, int w, bool fq) {
+    static const double f1[] = {0, .1234, .2440, .3559, .4380, .4379, .4409, .4420, .4430};
+    static const double q1[] = {0, .1157, .2300, .3373, .4266, .4433, .4576, .4600, .4623};
+    static const double f2[] = {0, .2455, .4575, .4650, .4665, .4672, .4675, .4678, .4680};
+    static const double q2[] = {0, .2283, .4310, .4580, .4626, .4626, .4630, .4632, .4634};
     if (w > 8) w = 8;
-    return fq ? on_q[w] : on_f[w];
+    if (w < 0) w = 0;
+    return ilp == 2 ? (fq ? q2[w] : f2[w]) : (fq ? q1[w] : f1[w]);
 }
 
 }  // namespace
 namespace lt_host {
-PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns) {
-    const unsigned long long groups = (n + 31) / 32;
+PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns, int max_ilp) {
     const int sms = tr->sm_count;
-    PersistentPlan best = {0, 4, 1, 512, 0, false};
+    PersistentPlan best = {0, 4, 1, 512, 0, false, 1};
     double best_score = -1.0;
-    for (int w = 1; w <= 16; ++w) {
-        if (w > 8 && (w & 1)) continue;                      // two CTAs per SM above 8
-        if (tr->warps_per_smsp > 0 && w != tr->warps_per_smsp) continue;
-        const unsigned long long slots = (unsigned long long)sms * 4 * w;
-        for (int fq = 0; fq < 2; ++fq) {
-            if (tr->flip_on_q >= 0 && fq != tr->flip_on_q) continue;
-            const double avg = (double)groups / ((double)sms * 4);   // groups per sub-partition
-            for (int dyn = 0; dyn < 2; ++dyn) {
-                double score;
-                if (dyn) {                                   // every slot busy until the tail
-                    if (groups <= slots && tr->fused_mode != 3) continue;
-                    score = loop_rate(w, fq);
-                } else if (groups <= slots) {                // one wave: busiest sub-partition rules
-                    const double per_smsp = std::ceil(avg);
-                    if (tr->warps_per_smsp == 0 && (double)w != std::min(per_smsp, 16.0)) continue;
-                    score = loop_rate((int)per_smsp, fq) * avg / per_smsp;
-                } else {                                     // static, several groups per slot in turn
-                    const double rounds = std::ceil((double)groups / (double)slots);
-                    score = loop_rate(w, fq) * avg / (rounds * w);
-                }
-                if (tr->fused_mode == 3 && !dyn) continue;
-                if (tr->fused_mode == 2 && dyn) continue;
-                if (score > best_score) {
-                    best_score = score;
-                    best.dynamic = dyn;
-                    best.warps_per_smsp = w;
-                    best.ctas_per_sm = w > 8 ? 2 : 1;
-                    best.threads = 128 * w / best.ctas_per_sm;
-                    best.flip_on_q = fq != 0;
+    for (int ilp = 1; ilp <= max_ilp; ++ilp) {
+        if (max_ilp > 1 && (tr->fused_ilp == 1 || tr->fused_ilp == 2) && ilp != tr->fused_ilp) continue;
+        const unsigned long long groups = (n + 32 * ilp - 1) / (32 * ilp);
+        const double avg = (double)groups / ((double)sms * 4);      // groups per sub-partition
+        for (int w = 1; w <= 16; ++w) {
+            if (w > 8 && (w & 1)) continue;                  // two CTAs per SM above 8
+            if (ilp == 2 && w > 4) continue;                 // 512 threads: 128 registers each
+            if (tr->warps_per_smsp > 0 && w != tr->warps_per_smsp) continue;
+            const unsigned long long slots = (unsigned long long)sms * 4 * w;
+            for (int fq = 0; fq < 2; ++fq) {
+                if (tr->flip_on_q >= 0 && fq != tr->flip_on_q) continue;
+                for (int dyn = 0; dyn < 2; ++dyn) {
+                    double score;
+                    if (dyn) {                               // every slot busy until the tail
+                        if (groups <= slots && tr->fused_mode != 3) continue;
+                        score = loop_rate(ilp, w, fq);
+                    } else if (groups <= slots) {            // one wave: busiest sub-partition rules
+                        const double per_smsp = std::ceil(avg);
+                        if (tr->warps_per_smsp == 0 && (double)w != std::min(per_smsp, ilp == 2 ? 4.0 : 16.0)) continue;
+                        score = loop_rate(ilp, (int)per_smsp, fq) * avg / per_smsp;
+                    } else {                                 // static, several groups per slot in turn
+                        const double rounds = std::ceil((double)groups / (double)slots);
+                        score = loop_rate(ilp, w, fq) * avg / (rounds * w);
+                    }
+                    if (tr->fused_mode == 3 && !dyn) continue;
+                    if (tr->fused_mode == 2 && dyn) continue;
+                    if (score > best_score) {
+                        best_score = score;
+                        best.dynamic = dyn;
+                        best.warps_per_smsp = w;
+                        best.ctas_per_sm = w > 8 ? 2 : 1;
+                        best.threads = 128 * w / best.ctas_per_sm;
+                        best.flip_on_q = fq != 0;
+                        best.ilp = ilp;
+                    }
                 }
             }
         }
     }
     if (best.dynamic) {
-        // long items amortise the ticket + L2 round trip (1024 turns: -0.5 %), short ones even
-        // out the tail: aim at >= 64 items per resident warp
+        // an item switch costs a warp about 3 us (ticket, progress word, state load; store, fence,
+        // release), during which its sub-partition runs at half rate when it holds two warps: long
+        // items (2048 turns = 120 us) amortise that, and the tapered tail of the schedule
+        // (ItemSchedule) keeps the last round short all the same (profiles/r2_item_sweep.md)
         unsigned long long it = tr->item_turns > 0
                                     ? (unsigned long long)tr->item_turns
-                                    : std::min<unsigned long long>(1024, std::max<unsigned long long>(256, turns / 64));
+                                    : std::min<unsigned long long>(2048, std::max<unsigned long long>(128, turns / 8));
         best.item_turns = (unsigned int)std::min<unsigned long long>(it, turns);
     } else {
         best.item_turns = 0;                                 // = all turns of the launch
@@ -274,18 +287,31 @@ PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long lon
 }  // namespace lt_host
 namespace {
 
+template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ, int ILP>
+cudaError_t launch_persistent_ilp(T* z, T* d, size_t n, unsigned int turns, unsigned int item_turns,
+                                  int first, int last, const PersistentPlan& pl, int sms,
+                                  unsigned long long* sched, const MapConsts<T>& c, cudaStream_t st) {
+    auto kern = fused_persistent_kernel<T, INTEG, HARM, SPLIT, FQ, false, ILP>;
+    // 1 CTA/SM: > half of the 227 KB; 2 CTAs/SM: > a third
+    const int smem = pl.ctas_per_sm == 1 ? 120 * 1024 : 80 * 1024;
+    static bool attr_set = false;                            // once per instantiation
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    kern<<<sms * pl.ctas_per_sm, pl.threads, smem, st>>>(z, d, n, turns, item_turns, first, last, pl.dynamic, sched,
+                                      reinterpret_cast<unsigned int*>(sched + 1), c, nullptr);
+    return cudaGetLastError();
+}
+
 template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ>
 cudaError_t launch_persistent_one(T* z, T* d, size_t n, unsigned int turns, unsigned int item_turns,
                                   int first, int last, const PersistentPlan& pl, int sms,
                                   unsigned long long* sched, const MapConsts<T>& c, cudaStream_t st) {
-    auto kern = fused_persistent_kernel<T, INTEG, HARM, SPLIT, FQ>;
-    // 1 CTA/SM: > half of the 227 KB; 2 CTAs/SM: > a third
-    const int smem = pl.ctas_per_sm == 1 ? 120 * 1024 : 80 * 1024;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    kern<<<sms * pl.ctas_per_sm, pl.threads, smem, st>>>(z, d, n, turns, item_turns, first, last, pl.dynamic, sched,
-                                      reinterpret_cast<unsigned int*>(sched + 1), c, nullptr);
-    return cudaGetLastError();
+    if (pl.ilp == 2)
+        return launch_persistent_ilp<T, INTEG, HARM, SPLIT, FQ, 2>(z, d, n, turns, item_turns, first, last, pl, sms, sched, c, st);
+    return launch_persistent_ilp<T, INTEG, HARM, SPLIT, FQ, 1>(z, d, n, turns, item_turns, first, last, pl, sms, sched, c, st);
 }
 
 template <typename T, int INTEG>
@@ -328,7 +354,7 @@ int track_fused_persistent(lt_tracker* tr, T* z, T* d, size_t n, unsigned long l
     int rc = ensure_sched(tr, n);
     if (rc) return rc;
     unsigned long long done = 0;
-    PersistentPlan pl = plan_persistent(tr, n, turns);
+    PersistentPlan pl = plan_persistent(tr, n, turns, 2);
     while (done < turns) {
         unsigned long long chunk = std::min<unsigned long long>(turns - done, (unsigned long long)tr->chunk_turns);
         const int first = done == 0, last = done + chunk == turns;
@@ -353,7 +379,7 @@ int track_fused_persistent(lt_tracker* tr, T* z, T* d, size_t n, unsigned long l
     }
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
-    tr->last_ilp = 1;
+    tr->last_ilp = pl.ilp;
     tr->last_mode = pl.dynamic ? 3 : 2;
     tr->last_item_turns = pl.dynamic ? pl.item_turns : 0;
     return LT_OK;
@@ -841,6 +867,85 @@ int lt_probe_fp64(int blocks, int threads, int chains, long long iters, double* 
     *rate_host = (double)blocks * threads * chains * (double)(iters / 16 * 16) / (ms * 1e-3);
     if (ms_host) *ms_host = ms;
     return LT_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+template <int CHAINS>
+cudaError_t launch_probe_pipe(int kind, int blocks, int threads, int iters, const ProbeConsts& P, double* out,
+                              unsigned long long* cyc, unsigned long long* ns) {
+#define LT_PP(K)                                                                                        \
+    case K: {                                                                                           \
+        auto kern = probe_pipe_kernel<CHAINS, K>;                                                       \
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024); \
+        if (e != cudaSuccess) return e;                                                                 \
+        kern<<<blocks, threads, 120 * 1024>>>(out, iters, P, cyc, ns);                                  \
+        return cudaGetLastError();                                                                      \
+    }
+    switch (kind) {
+        LT_PP(0) LT_PP(1) LT_PP(2) LT_PP(3) LT_PP(10) LT_PP(11) LT_PP(12)
+        default: return cudaErrorInvalidValue;
+    }
+#undef LT_PP
+}
+
+}  // namespace
+
+extern "C" {
+
+int lt_probe_pipe(int kind, int blocks, int threads, int chains, long long iters,
+                  double* instr_per_cycle_host, double* sm_clock_mhz_host) {
+    if (!instr_per_cycle_host) return LT_E_NULL;
+    if (blocks < 1 || blocks > 1024 || threads < 32 || threads > 1024 || (threads & 31) || iters < 1 ||
+        iters > (1LL << 28))
+        return LT_E_PARAM;
+    if (chains != 1 && chains != 2 && chains != 4) return LT_E_PARAM;
+    if (kind != 0 && kind != 1 && kind != 2 && kind != 3 && kind != 10 && kind != 11 && kind != 12) return LT_E_PARAM;
+    ProbeConsts P;
+    for (int k = 0; k < 8; ++k) P.c[k] = (double)(7.6973252442360035e-5L * LT_SINPI_F64[k]);
+    P.drift = 5.7; P.a = 0.999999; P.b = 1e-6;
+    double* out = nullptr;
+    unsigned long long* cyc = nullptr;
+    if (cudaMalloc(&out, sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&cyc, 2 * sizeof(unsigned long long) * (size_t)blocks) != cudaSuccess) {
+        (void)cudaGetLastError();
+        if (out) cudaFree(out);
+        return LT_E_CUDA;
+    }
+    unsigned long long* ns = cyc + blocks;
+    cudaError_t e = cudaSuccess;
+    for (int rep = 0; rep < 2 && e == cudaSuccess; ++rep) {     // first repetition warms up
+        e = chains == 1 ? launch_probe_pipe<1>(kind, blocks, threads, (int)iters, P, out, cyc, ns)
+          : chains == 2 ? launch_probe_pipe<2>(kind, blocks, threads, (int)iters, P, out, cyc, ns)
+                        : launch_probe_pipe<4>(kind, blocks, threads, (int)iters, P, out, cyc, ns);
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    }
+    int rc = LT_OK;
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        rc = LT_E_CUDA;
+    } else {
+        unsigned long long* h = (unsigned long long*)std::malloc(2 * sizeof(unsigned long long) * (size_t)blocks);
+        if (!h) rc = LT_E_NOMEM;
+        else if (cudaMemcpy(h, cyc, 2 * sizeof(unsigned long long) * (size_t)blocks, cudaMemcpyDeviceToHost) != cudaSuccess) {
+            (void)cudaGetLastError();
+            rc = LT_E_CUDA;
+        } else {
+            double mc = 0.0, mn = 0.0;
+            for (int i = 0; i < blocks; ++i) { mc += (double)h[i]; mn += (double)h[blocks + i]; }
+            mc /= blocks; mn /= blocks;
+            const double per = kind >= 10 ? 13.0 : 1.0;        // FP64 instructions per step and chain
+            const double warp_instr_per_smsp = (threads / 32) / 4.0 * chains * 8.0 * (double)iters * per;
+            *instr_per_cycle_host = warp_instr_per_smsp / mc;
+            if (sm_clock_mhz_host) *sm_clock_mhz_host = mn > 0.0 ? mc / mn * 1e3 : 0.0;
+        }
+        std::free(h);
+    }
+    cudaFree(out);
+    cudaFree(cyc);
+    return rc;
 }
 
 }  // extern "C"

@@ -26,19 +26,35 @@ int residency_smem(const PersistentPlan& pl) {
 // ------------------------------------------------------------------------------------------
 // f2, fused mode: the persistent kernel with PROG, one packed table per launch
 // ------------------------------------------------------------------------------------------
+template <int INTEG, int HARM, bool SPLIT, bool FQ, int ILP>
+cudaError_t launch_prog_ilp(double* z, double* d, size_t n, unsigned int turns, unsigned int item_turns,
+                            int first, int last, const PersistentPlan& pl, int sms,
+                            unsigned long long* sched, const MapConsts<double>& c,
+                            const double2* prog, cudaStream_t st) {
+    auto kern = fused_persistent_kernel<double, INTEG, HARM, SPLIT, FQ, true, ILP>;
+    const int smem = residency_smem(pl);                     // >= 512 B of staged entries per warp
+    static bool attr_set = false;                            // once per instantiation
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    kern<<<sms * pl.ctas_per_sm, pl.threads, smem, st>>>(z, d, n, turns, item_turns, first, last,
+                                                         pl.dynamic, sched,
+                                                         reinterpret_cast<unsigned int*>(sched + 1), c, prog);
+    return cudaGetLastError();
+}
+
 template <int INTEG, int HARM, bool SPLIT>
 cudaError_t launch_prog_one(double* z, double* d, size_t n, unsigned int turns, unsigned int item_turns,
                             int first, int last, const PersistentPlan& pl, int sms,
                             unsigned long long* sched, const MapConsts<double>& c,
                             const double2* prog, cudaStream_t st) {
-    auto kern = fused_persistent_kernel<double, INTEG, HARM, SPLIT, !SPLIT, true>;
-    const int smem = residency_smem(pl);
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    kern<<<sms * pl.ctas_per_sm, pl.threads, smem, st>>>(z, d, n, turns, item_turns, first, last,
-                                                         pl.dynamic, sched,
-                                                         reinterpret_cast<unsigned int*>(sched + 1), c, prog);
-    return cudaGetLastError();
+#define LT_PI(Q, I) launch_prog_ilp<INTEG, HARM, SPLIT, Q, I>(z, d, n, turns, item_turns, first, last, pl, sms, sched, c, prog, st)
+    if (SPLIT || HARM == 0) return pl.ilp == 2 ? LT_PI(false, 2) : LT_PI(false, 1);
+    if (pl.ilp == 2) return pl.flip_on_q ? LT_PI(true, 2) : LT_PI(false, 2);
+    return pl.flip_on_q ? LT_PI(true, 1) : LT_PI(false, 1);
+#undef LT_PI
 }
 
 template <int INTEG>
@@ -71,10 +87,10 @@ int track_programme_fused(lt_tracker* tr, double* z, double* d, size_t n, unsign
     const size_t want = (size_t)std::min<unsigned long long>(turns, chunk_max);
     if (tr->prog_entries < want) {
         if (tr->prog_table) { LT_CUDA(tr, cudaFree(tr->prog_table)); tr->prog_table = nullptr; tr->prog_entries = 0; }
-        LT_CUDA(tr, cudaMalloc(&tr->prog_table, want * sizeof(double2)));
+        LT_CUDA(tr, cudaMalloc(&tr->prog_table, (want + 1) * sizeof(double2)));   // + the header entry
         tr->prog_entries = want;
     }
-    const PersistentPlan pl = plan_persistent(tr, n, turns);
+    const PersistentPlan pl = plan_persistent(tr, n, turns, 2);
     unsigned long long done = 0;
     while (done < turns) {
         const unsigned long long chunk = std::min<unsigned long long>(turns - done, chunk_max);
@@ -83,19 +99,19 @@ int track_programme_fused(lt_tracker* tr, double* z, double* d, size_t n, unsign
                                              : (unsigned int)chunk;
         // the table of the previous chunk is free again: its kernel precedes this one on the stream
         programme_pack_kernel<<<(unsigned)((chunk + 255) / 256), 256, 0, st>>>(
-            volt + done, phase + done, (unsigned int)chunk, kInvPi, tr->prog_table);
+            volt, phase, done, (unsigned int)chunk, turns, kInvPi, split ? 0 : 1, tr->prog_table);
         LT_CUDA(tr, cudaGetLastError());
         if (pl.dynamic) LT_CUDA(tr, cudaMemsetAsync(tr->sched, 0, 8 + 4 * ((n + 31) / 32), st));
         cudaError_t e;
         switch (tr->p.integrator) {
             case LT_EULER_CROMER:
-                e = launch_prog_integ<kEulerCromer>(tr->harm, split, z, d, n, (unsigned)chunk, item, first, last, pl, tr->sm_count, tr->sched, tr->c64, tr->prog_table, st);
+                e = launch_prog_integ<kEulerCromer>(tr->harm, split, z, d, n, (unsigned)chunk, item, first, last, pl, tr->sm_count, tr->sched, tr->c64, tr->prog_table + 1, st);
                 break;
             case LT_LEAPFROG:
-                e = launch_prog_integ<kLeapfrog>(tr->harm, split, z, d, n, (unsigned)chunk, item, first, last, pl, tr->sm_count, tr->sched, tr->c64, tr->prog_table, st);
+                e = launch_prog_integ<kLeapfrog>(tr->harm, split, z, d, n, (unsigned)chunk, item, first, last, pl, tr->sm_count, tr->sched, tr->c64, tr->prog_table + 1, st);
                 break;
             default:
-                e = launch_prog_integ<kRuth4>(tr->harm, split, z, d, n, (unsigned)chunk, item, first, last, pl, tr->sm_count, tr->sched, tr->c64, tr->prog_table, st);
+                e = launch_prog_integ<kRuth4>(tr->harm, split, z, d, n, (unsigned)chunk, item, first, last, pl, tr->sm_count, tr->sched, tr->c64, tr->prog_table + 1, st);
         }
         LT_CUDA(tr, e);
         tr->launches += 2;
@@ -103,7 +119,7 @@ int track_programme_fused(lt_tracker* tr, double* z, double* d, size_t n, unsign
     }
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
-    tr->last_ilp = 1;
+    tr->last_ilp = pl.ilp;
     tr->last_mode = pl.dynamic ? 3 : 2;
     tr->last_item_turns = pl.dynamic ? pl.item_turns : 0;
     return LT_OK;
@@ -303,12 +319,12 @@ TransPlan plan_transverse(const lt_tracker* tr, size_t n, unsigned long long tur
     }
     tp.ilp = ilp;
     const unsigned long long groups = (n + 32 * ilp - 1) / (32 * ilp);
-    PersistentPlan pl = {0, 4, 1, 512, 0, true};
+    PersistentPlan pl = {0, 4, 1, 512, 0, true, 1};
     pl.dynamic = (groups > slots || tr->fused_mode == 3) && tr->fused_mode != 2;
     if (pl.dynamic) {
         unsigned long long it = tr->item_turns > 0
                                     ? (unsigned long long)tr->item_turns
-                                    : std::min<unsigned long long>(1024, std::max<unsigned long long>(256, turns / 64));
+                                    : std::min<unsigned long long>(2048, std::max<unsigned long long>(128, turns / 8));
         pl.item_turns = (unsigned int)std::min<unsigned long long>(it, turns);
     }
     tp.pl = pl;

@@ -54,20 +54,34 @@ int check_args(const lt_tracker* tr, const double* z, const double* d, size_t n,
     return LT_OK;
 }
 
+template <int HARM, bool SPLIT, int ILP>
+cudaError_t launch_ramp_fused_ilp(double* z, double* d, size_t n, unsigned int nsteps, unsigned int item_steps,
+                                  int first, int last, const PersistentPlan& pl, const lt_tracker* tr,
+                                  cudaStream_t st) {
+    auto kern = ramp_persistent_kernel<HARM, SPLIT, ILP>;
+    // the request caps the CTAs per SM (1 CTA/SM: > half of the 227 KB; 2 CTAs/SM: > a third) and
+    // holds 3072 B of staging per warp: 32 warps of a 2-CTA launch need 96 KB, which still fits twice
+    const int warps = pl.threads / 32;
+    const int smem = std::max(pl.ctas_per_sm == 1 ? 120 * 1024 : 80 * 1024, warps * 3072);
+    static bool attr_set = false;                            // once per instantiation
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    kern<<<tr->sm_count * pl.ctas_per_sm, pl.threads, smem, st>>>(
+        z, d, n, nsteps, item_steps, first, last, pl.dynamic, tr->sched,
+        reinterpret_cast<unsigned int*>(tr->sched + 1), tr->c64,
+        reinterpret_cast<const double2*>(reinterpret_cast<const RampEntry*>(tr->ramp_table) + (SPLIT ? 0 : 1)));
+    return cudaGetLastError();
+}
+
 template <int HARM, bool SPLIT>
 cudaError_t launch_ramp_fused(double* z, double* d, size_t n, unsigned int nsteps, unsigned int item_steps,
                               int first, int last, const PersistentPlan& pl, const lt_tracker* tr,
                               cudaStream_t st) {
-    auto kern = ramp_persistent_kernel<HARM, SPLIT>;
-    // 1 CTA/SM: > half of the 227 KB; 2 CTAs/SM: > a third (and >= 1536 B per warp of staging)
-    const int smem = pl.ctas_per_sm == 1 ? 120 * 1024 : 80 * 1024;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    kern<<<tr->sm_count * pl.ctas_per_sm, pl.threads, smem, st>>>(
-        z, d, n, nsteps, item_steps, first, last, pl.dynamic, tr->sched,
-        reinterpret_cast<unsigned int*>(tr->sched + 1), tr->c64,
-        reinterpret_cast<const double2*>(tr->ramp_table));
-    return cudaGetLastError();
+    if (pl.ilp == 2) return launch_ramp_fused_ilp<HARM, SPLIT, 2>(z, d, n, nsteps, item_steps, first, last, pl, tr, st);
+    return launch_ramp_fused_ilp<HARM, SPLIT, 1>(z, d, n, nsteps, item_steps, first, last, pl, tr, st);
 }
 
 template <int HARM, int NSUB>
@@ -135,9 +149,9 @@ int lt_track_ramp(lt_tracker* tr, double* z, double* d, size_t n, unsigned long 
     const bool split = tr->split_drifts != 0;
     const unsigned long long chunk_max =
         std::min<unsigned long long>((unsigned long long)tr->chunk_turns, kRampChunkMax);
-    rc = ensure_ramp_table(tr, (size_t)std::min<unsigned long long>(turns, chunk_max) * nsub);
+    rc = ensure_ramp_table(tr, (size_t)std::min<unsigned long long>(turns, chunk_max) * nsub + 1);   // + header
     if (rc) return rc;
-    const PersistentPlan pl = plan_persistent(tr, n, turns);
+    const PersistentPlan pl = plan_persistent(tr, n, turns, 2);
     const RampRing R = make_ring(tr);
     unsigned long long done = 0;
     while (done < turns) {
@@ -165,7 +179,7 @@ int lt_track_ramp(lt_tracker* tr, double* z, double* d, size_t n, unsigned long 
     }
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
-    tr->last_ilp = 1;
+    tr->last_ilp = pl.ilp;
     tr->last_mode = pl.dynamic ? 3 : 2;
     tr->last_item_turns = pl.dynamic ? pl.item_turns : 0;
     return LT_OK;

@@ -41,6 +41,7 @@ struct PersistentPlan {
     int dynamic, warps_per_smsp, ctas_per_sm, threads;
     unsigned int item_turns;
     bool flip_on_q;
+    int ilp;                  // particles per lane of the persistent kernel (1 or 2)
 };
 
 }  // namespace lt_host
@@ -102,7 +103,8 @@ inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
 int ensure_device(lt_tracker* tr);
 int ensure_scratch(lt_tracker* tr, int grid);
 int ensure_sched(lt_tracker* tr, size_t n);
-PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns);
+// max_ilp: 2 where the kernel has a two-particles-per-lane instantiation, else 1
+PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns, int max_ilp = 1);
 int per_turn_grid(const lt_tracker* tr, size_t n);
 // the BASELINE path's fused / per-turn entry points, for calls that compose with them
 int track_fused_f64(lt_tracker* tr, double* z, double* d, size_t n, unsigned long long turns,

@@ -89,6 +89,8 @@ def _load():
         "lt_track_fused_host": (c_int, [vp, vp, vp, sz, ull, POINTER(ull)]),
         "lt_probe_fp64": (c_int, [c_int, c_int, c_int, c_longlong, POINTER(c_double),
                                   POINTER(c_double)]),
+        "lt_probe_pipe": (c_int, [c_int, c_int, c_int, c_int, c_longlong, POINTER(c_double),
+                                  POINTER(c_double)]),
         # SURVEY.md sec. 8(f) rows f2-f4
         "lt_track_programme": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp]),
         "lt_track_programme_per_turn": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp, vp, vp]),
@@ -276,6 +278,15 @@ def probe_fp64(blocks: int, threads: int, chains: int, iters: int):
     if rc != OK:
         raise LongtrackError(rc)
     return rate.value, ms.value
+
+
+def probe_pipe(kind: int, blocks: int, threads: int, chains: int, iters: int):
+    """Returns (FP64 warp-instructions per cycle per sub-partition, SM clock in MHz)."""
+    rate, mhz = c_double(), c_double()
+    rc = _lib.lt_probe_pipe(kind, blocks, threads, chains, iters, byref(rate), byref(mhz))
+    if rc != OK:
+        raise LongtrackError(rc)
+    return rate.value, mhz.value
 
 
 def strerror(code: int) -> str:
