@@ -38,7 +38,11 @@ struct TurnExtras {
 };
 
 // CTA-private histogram in shared memory, `replicas` copies indexed by lane so that the
-// particles of one warp that fall into the same slice do not serialise on one address.
+// particles of one warp that fall into the same slice do not serialise on one address (a
+// Gaussian bunch puts 40 % of the particles into the 10 central slices of 64).  Copy-major with
+// an odd stride; a counter-major layout (bank = lane, no bank conflicts at all) measured no
+// faster: the kernel is bound by its loads, not by the shared atomics
+// (profiles/r2_histogram.md).
 struct SliceAcc {
     unsigned int* sh;
     unsigned long long* out;
@@ -182,35 +186,76 @@ static __global__ void advance_cursor_kernel(unsigned long long* cursor, unsigne
     *cursor += by;
 }
 
-// Histogram of a given state (lt_slice_histogram): 8 B read per particle.  Persistent CTAs walk
-// tiles of blockDim.x * 2 * UNR particles; the UNR 16-byte loads of a tile are all issued before
-// the first shared-memory atomic, so that every thread keeps 64 B in flight (one 8-byte load per
-// grid-stride step left the kernel latency-bound at 35 % of the copy rate).  A z array that is
-// only 8-byte aligned is shifted by one element (`head`), which the first thread takes alone.
+// Histogram of a given state (lt_slice_histogram): 8 B read per particle, HBM bound.
+// One wave of persistent CTAs (grid = a multiple of the SM count, 512 threads); every thread
+// keeps TWO tiles of UNR 16-byte loads in flight: the loads of tile k+1 are issued before the
+// shared-memory atomics of tile k (128 B per thread; the first version issued a tile's loads only
+// after the previous tile's atomics and ran 1184 short-lived CTAs whose zero / load / flush
+// phases coincided: 3.7 TB/s in the kernel, profiles/r1_next_rows_ncu.md).
+// No memset launch: the CTAs add their counts into a tracker-owned accumulator `acc` that is
+// zero between calls; the last CTA to finish (ticket in *arrived) copies it over the caller's
+// histogram and zeroes it again.  acc == nullptr: the counts go straight into `out`, which the
+// caller zeroed (more slices than the shared-memory path holds).
+// A z array that is only 8-byte aligned is shifted by one element (`head`).
 template <int UNR>
-static __global__ void slice_histogram_kernel(const double* __restrict__ z_arr, size_t n,
-                                       const __grid_constant__ TurnExtras X) {
+static __global__ void __launch_bounds__(512)
+slice_histogram_kernel(const double* __restrict__ z_arr, size_t n, const __grid_constant__ TurnExtras X,
+                       unsigned long long* __restrict__ acc, unsigned int* __restrict__ arrived) {
     extern __shared__ unsigned int slice_smem[];
+    __shared__ int is_last;
     SliceAcc sl;
     sl.init(X, 0ULL, slice_smem);
+    unsigned long long* const out = sl.out;
+    if (acc) sl.out = acc;
     const size_t head = ((reinterpret_cast<uintptr_t>(z_arr) & 15u) != 0 && n > 0) ? 1 : 0;
     if (head && blockIdx.x == 0 && threadIdx.x == 0) sl.add(z_arr[0]);
     const double* __restrict__ zb = z_arr + head;
     const size_t m = n - head;
     const size_t tile = (size_t)blockDim.x * 2 * UNR;
-    for (size_t base = (size_t)blockIdx.x * tile; base < m; base += (size_t)gridDim.x * tile) {
-        double2 v[UNR];
-        if (base + tile <= m) {
+    const size_t stride = (size_t)gridDim.x * tile;
+    size_t base = (size_t)blockIdx.x * tile;
+    double2 cur[UNR];
+    bool have = base + tile <= m;
+    if (have) {
+#pragma unroll
+        for (int u = 0; u < UNR; ++u)
+            cur[u] = __ldcs(reinterpret_cast<const double2*>(zb + base) + u * blockDim.x + threadIdx.x);
+    }
+    while (have) {
+        const size_t nb = base + stride;
+        const bool more = nb + tile <= m;
+        double2 nxt[UNR];
+        if (more) {
 #pragma unroll
             for (int u = 0; u < UNR; ++u)
-                v[u] = __ldcs(reinterpret_cast<const double2*>(zb + base) + u * blockDim.x + threadIdx.x);
-#pragma unroll
-            for (int u = 0; u < UNR; ++u) { sl.add(v[u].x); sl.add(v[u].y); }
-        } else {
-            for (size_t i = base + threadIdx.x; i < m; i += blockDim.x) sl.add(zb[i]);
+                nxt[u] = __ldcs(reinterpret_cast<const double2*>(zb + nb) + u * blockDim.x + threadIdx.x);
         }
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) { sl.add(cur[u].x); sl.add(cur[u].y); }
+#pragma unroll
+        for (int u = 0; u < UNR; ++u) cur[u] = nxt[u];
+        base = nb;
+        have = more;
+    }
+    // `base` is this CTA's first tile that is not full: at most one ragged tile in the whole grid
+    for (size_t i = base + threadIdx.x; i < m && base < m; i += blockDim.x) {
+        if (i < base + tile) sl.add(zb[i]);
     }
     sl.flush();
+    if (acc) {
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) is_last = atomicAdd(arrived, 1u) == gridDim.x - 1;
+        __syncthreads();
+        if (is_last) {
+            __threadfence();
+            for (int b = threadIdx.x; b < X.n_slices + 2; b += blockDim.x) {
+                out[b] = __ldcg(acc + b);
+                acc[b] = 0ULL;
+            }
+            if (threadIdx.x == 0) *arrived = 0u;
+        }
+    }
 }
 
 // Programme table of one fused launch, double2 per turn behind a one-entry header:

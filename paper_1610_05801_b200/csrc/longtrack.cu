@@ -118,18 +118,18 @@ namespace {
 
 }  // namespace
 namespace lt_host {
-int ensure_scratch(lt_tracker* tr, int grid) {
+int ensure_scratch(lt_tracker* tr, int grid, cudaStream_t st) {
     const size_t need = (size_t)kBatchTurns * (size_t)grid * kPartialStride;
     if (tr->partials_doubles < need) {
         // the cached per-turn graph has the old scratch address baked in
         if (tr->graph_exec) { cudaGraphExecDestroy(tr->graph_exec); tr->graph_exec = nullptr; }
-        if (tr->partials) { LT_CUDA(tr, cudaFree(tr->partials)); tr->partials = nullptr; tr->partials_doubles = 0; }
-        LT_CUDA(tr, cudaMalloc(&tr->partials, need * sizeof(double)));
+        size_t have = tr->partials_doubles * sizeof(double);
+        LT_CUDA(tr, grow_async((void**)&tr->partials, &have, need * sizeof(double), st));
         tr->partials_doubles = need;
     }
     if (!tr->cursor) {
-        LT_CUDA(tr, cudaMalloc(&tr->cursor, 2 * sizeof(unsigned long long)));
-        LT_CUDA(tr, cudaMemset(tr->cursor, 0, 2 * sizeof(unsigned long long)));
+        LT_CUDA(tr, cudaMallocAsync((void**)&tr->cursor, 2 * sizeof(unsigned long long), st));
+        LT_CUDA(tr, cudaMemsetAsync(tr->cursor, 0, 2 * sizeof(unsigned long long), st));
     }
     return LT_OK;
 }
@@ -332,14 +332,10 @@ cudaError_t launch_persistent_integ(int harm, bool split, T* z, T* d, size_t n, 
 
 }  // namespace
 namespace lt_host {
-int ensure_sched(lt_tracker* tr, size_t n) {
+int ensure_sched(lt_tracker* tr, size_t n, cudaStream_t st) {
     const size_t groups = (n + 31) / 32;
     const size_t need = 8 + 4 * groups + 8;
-    if (tr->sched_bytes < need) {
-        if (tr->sched) { LT_CUDA(tr, cudaFree(tr->sched)); tr->sched = nullptr; tr->sched_bytes = 0; }
-        LT_CUDA(tr, cudaMalloc(&tr->sched, need));
-        tr->sched_bytes = need;
-    }
+    LT_CUDA(tr, grow_async((void**)&tr->sched, &tr->sched_bytes, need, st));
     return LT_OK;
 }
 }  // namespace lt_host
@@ -351,7 +347,7 @@ int track_fused_persistent(lt_tracker* tr, T* z, T* d, size_t n, unsigned long l
     const MapConsts<T>& c = *reinterpret_cast<const MapConsts<T>*>(
         sizeof(T) == 8 ? (const void*)&tr->c64 : (const void*)&tr->c32);
     const bool split = tr->split_drifts != 0 || tr->harm == 0;
-    int rc = ensure_sched(tr, n);
+    int rc = ensure_sched(tr, n, st);
     if (rc) return rc;
     unsigned long long done = 0;
     PersistentPlan pl = plan_persistent(tr, n, turns, 2);
@@ -516,7 +512,7 @@ int track_per_turn(lt_tracker* tr, T* z, T* d, size_t n, unsigned long long turn
     const int grid = per_turn_grid(tr, n);
     cudaStream_t st = (cudaStream_t)stream;
     if (moments) {
-        rc = ensure_scratch(tr, grid);
+        rc = ensure_scratch(tr, grid, st);
         if (rc) return rc;
         set_cursor_kernel<<<1, 1, 0, st>>>(tr->cursor, reinterpret_cast<unsigned int*>(tr->cursor + 1), 0ULL);
         LT_CUDA(tr, cudaGetLastError());
@@ -537,8 +533,10 @@ int track_per_turn(lt_tracker* tr, T* z, T* d, size_t n, unsigned long long turn
             cudaError_t e = enqueue_batch<T>(tr, z, d, n, 0, kBatchTurns, moments, mo, so, vec_ok, grid, c, tr->capture_stream);
             tr->launches = before;      // capture enqueues nothing
             cudaError_t e2 = cudaStreamEndCapture(tr->capture_stream, &graph);
-            LT_CUDA(tr, e);
-            LT_CUDA(tr, e2);
+            if (e != cudaSuccess || e2 != cudaSuccess) {        // no graph is left behind on failure
+                if (graph) cudaGraphDestroy(graph);
+                LT_CUDA(tr, e != cudaSuccess ? e : e2);
+            }
             cudaError_t e3 = cudaGraphInstantiate(&tr->graph_exec, graph, 0);
             cudaGraphDestroy(graph);
             LT_CUDA(tr, e3);
@@ -573,7 +571,7 @@ int state_sums(lt_tracker* tr, const T* z, const T* d, size_t n, lt_moments* mo,
     size_t g = (n + 255) / 256;
     if (g > (size_t)tr->sm_count * 8) g = (size_t)tr->sm_count * 8;
     if (g < 1) g = 1;
-    rc = ensure_scratch(tr, (int)g);
+    rc = ensure_scratch(tr, (int)g, st);
     if (rc) return rc;
     state_sums_kernel<T, ONLY_COUNT><<<(unsigned)g, 256, 0, st>>>(z, d, n, tr->partials, c);
     LT_CUDA(tr, cudaGetLastError());

@@ -78,17 +78,17 @@ int track_programme_fused(lt_tracker* tr, double* z, double* d, size_t n, unsign
     if (n > ((size_t)1 << 40)) return LT_E_PARAM;
     int rc = ensure_device(tr);
     if (rc) return rc;
-    rc = ensure_sched(tr, n);
-    if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    rc = ensure_sched(tr, n, st);
+    if (rc) return rc;
     const bool split = tr->split_drifts != 0 || tr->harm == 0;
     const unsigned long long chunk_max =
         std::min<unsigned long long>((unsigned long long)tr->chunk_turns, kProgChunkMax);
     const size_t want = (size_t)std::min<unsigned long long>(turns, chunk_max);
-    if (tr->prog_entries < want) {
-        if (tr->prog_table) { LT_CUDA(tr, cudaFree(tr->prog_table)); tr->prog_table = nullptr; tr->prog_entries = 0; }
-        LT_CUDA(tr, cudaMalloc(&tr->prog_table, (want + 1) * sizeof(double2)));   // + the header entry
-        tr->prog_entries = want;
+    {
+        size_t have = tr->prog_entries ? (tr->prog_entries + 1) * sizeof(double2) : 0;
+        LT_CUDA(tr, grow_async((void**)&tr->prog_table, &have, (want + 1) * sizeof(double2), st));   // + the header entry
+        if (tr->prog_entries < want) tr->prog_entries = want;
     }
     const PersistentPlan pl = plan_persistent(tr, n, turns, 2);
     unsigned long long done = 0;
@@ -137,14 +137,17 @@ struct ExtraArgs {
 
 size_t slice_stride(int n_slices) { return ((size_t)n_slices + 2) | 1; }
 
-// shared-memory copies of the histogram
+// shared-memory copies of the histogram: one per lane when they fit (no two lanes of a warp ever
+// share a counter), halved until the copies fit 32 KB per CTA; 0 = global atomics
 int slice_replicas(int n_slices) {
-    // one copy per lane when they fit (no two lanes of a warp ever share a counter), halved until
-    // the copies fit 32 KB per CTA; the stride is made odd (see SliceAcc)
     const size_t one = slice_stride(n_slices) * sizeof(unsigned int);
     int r = 32;
     while (r > 0 && (size_t)r * one > 32 * 1024) r >>= 1;
     return r;
+}
+
+size_t slice_smem_bytes(const TurnExtras& X) {
+    return (size_t)X.replicas * slice_stride(X.n_slices) * sizeof(unsigned int);
 }
 
 TurnExtras make_extras(const lt_tracker* tr, const ExtraArgs& a, int k) {
@@ -169,7 +172,7 @@ template <int INTEG, int HARM>
 cudaError_t launch_extra_one(double* z, double* d, size_t n, int reverse, double* partials,
                              bool moments, bool vec_ok, int grid, const MapConsts<double>& c,
                              const TurnExtras& X, cudaStream_t st) {
-    const size_t smem = (size_t)X.replicas * slice_stride(X.n_slices) * sizeof(unsigned int);
+    const size_t smem = slice_smem_bytes(X);
     if (vec_ok) {
         if (moments)
             per_turn_extra_kernel<INTEG, HARM, true, kPerTurnUnroll><<<grid, kPerTurnThreads, smem, st>>>(z, d, n, reverse, partials, c, X);
@@ -243,7 +246,7 @@ int track_per_turn_extra(lt_tracker* tr, double* z, double* d, size_t n, unsigne
     const bool moments = mo || so;
     const bool vec_ok = aligned(z, 16) && aligned(d, 16);
     const int grid = per_turn_grid(tr, n);
-    rc = ensure_scratch(tr, grid);
+    rc = ensure_scratch(tr, grid, st);
     if (rc) return rc;
     set_cursor_kernel<<<1, 1, 0, st>>>(tr->cursor, reinterpret_cast<unsigned int*>(tr->cursor + 1), 0ULL);
     LT_CUDA(tr, cudaGetLastError());
@@ -263,8 +266,10 @@ int track_per_turn_extra(lt_tracker* tr, double* z, double* d, size_t n, unsigne
             cudaError_t e = enqueue_extra_batch(tr, z, d, n, 0, kBatchTurns, moments, mo, so, vec_ok, grid, a, tr->capture_stream);
             tr->launches = before;      // capture enqueues nothing
             cudaError_t e2 = cudaStreamEndCapture(tr->capture_stream, &graph);
-            LT_CUDA(tr, e);
-            LT_CUDA(tr, e2);
+            if (e != cudaSuccess || e2 != cudaSuccess) {        // no graph is left behind on failure
+                if (graph) cudaGraphDestroy(graph);
+                LT_CUDA(tr, e != cudaSuccess ? e : e2);
+            }
             cudaError_t e3 = cudaGraphInstantiate(&tr->graph_exec, graph, 0);
             cudaGraphDestroy(graph);
             LT_CUDA(tr, e3);
@@ -289,7 +294,7 @@ int track_per_turn_extra(lt_tracker* tr, double* z, double* d, size_t n, unsigne
 // ------------------------------------------------------------------------------------------
 int ensure_lattice(lt_tracker* tr, cudaStream_t st) {
     if (tr->n_seg <= 0 || !tr->lattice_host) return LT_E_PARAM;   // lt_set_transverse not called
-    if (!tr->lattice_dev) LT_CUDA(tr, cudaMalloc(&tr->lattice_dev, (size_t)kMaxSegments * 16 * sizeof(double)));
+    if (!tr->lattice_dev) LT_CUDA(tr, cudaMallocAsync((void**)&tr->lattice_dev, (size_t)kMaxSegments * 16 * sizeof(double), st));
     if (tr->lattice_dirty) {
         // pageable source: the copy is staged before the call returns and ordered on the stream
         LT_CUDA(tr, cudaMemcpyAsync(tr->lattice_dev, tr->lattice_host, (size_t)tr->n_seg * 16 * sizeof(double),
@@ -398,7 +403,7 @@ int track_transverse_fused(lt_tracker* tr, double* x, double* xp, double* y, dou
     cudaStream_t st = (cudaStream_t)stream;
     rc = ensure_lattice(tr, st);
     if (rc) return rc;
-    rc = ensure_sched(tr, n);
+    rc = ensure_sched(tr, n, st);
     if (rc) return rc;
     const bool longi = z && longitudinal_rides_along(tr, true);
     const TransPlan tp = plan_transverse(tr, n, turns);
@@ -470,6 +475,7 @@ int track_transverse_per_turn(lt_tracker* tr, double* x, double* xp, double* y, 
 namespace lt_host {
 void destroy_next(lt_tracker* tr) {
     if (tr->prog_table) cudaFree(tr->prog_table);
+    if (tr->hist_acc) cudaFree(tr->hist_acc);
     if (tr->lattice_dev) cudaFree(tr->lattice_dev);
     std::free(tr->lattice_host);
 }
@@ -520,15 +526,25 @@ int lt_slice_histogram(lt_tracker* tr, const double* z_dev, size_t n, double z_l
     int rc = ensure_device(tr);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    LT_CUDA(tr, cudaMemsetAsync(hist_dev, 0, ((size_t)n_slices + 2) * sizeof(unsigned long long), st));
-    if (n == 0) return LT_OK;
     const ExtraArgs a = {nullptr, nullptr, hist_dev, z_lo, z_hi, n_slices};
     const TurnExtras X = make_extras(tr, a, 0);
-    constexpr int kUnr = 4;                                   // 64 B in flight per thread
-    size_t g = (n + 256 * 2 * kUnr - 1) / (256 * 2 * kUnr);
-    g = std::max<size_t>(1, std::min<size_t>(g, (size_t)tr->sm_count * 8));
-    const size_t smem = (size_t)X.replicas * slice_stride(n_slices) * sizeof(unsigned int);
-    slice_histogram_kernel<kUnr><<<(unsigned)g, 256, smem, st>>>(z_dev, n, X);
+    const bool direct = X.replicas == 0 || n == 0;           // counts straight into hist_dev
+    if (direct) {
+        LT_CUDA(tr, cudaMemsetAsync(hist_dev, 0, ((size_t)n_slices + 2) * sizeof(unsigned long long), st));
+        if (n == 0) return LT_OK;
+    } else if (!tr->hist_acc) {
+        // accumulator of the shared-memory path (<= 8190 slices) + the arrival ticket, zero between calls
+        const size_t bytes = (size_t)(kMaxSharedSlices + 2 + 1) * sizeof(unsigned long long);
+        LT_CUDA(tr, cudaMallocAsync((void**)&tr->hist_acc, bytes, st));
+        LT_CUDA(tr, cudaMemsetAsync(tr->hist_acc, 0, bytes, st));
+    }
+    constexpr int kUnr = 4, kThreads = 512;                   // 2 x 64 B in flight per thread
+    size_t g = (n + kThreads * 2 * kUnr - 1) / (kThreads * 2 * kUnr);
+    g = std::max<size_t>(1, std::min<size_t>(g, (size_t)tr->sm_count * 2));
+    const size_t smem = slice_smem_bytes(X);
+    unsigned long long* acc = direct ? nullptr : tr->hist_acc;
+    slice_histogram_kernel<kUnr><<<(unsigned)g, kThreads, smem, st>>>(
+        z_dev, n, X, acc, reinterpret_cast<unsigned int*>(tr->hist_acc ? tr->hist_acc + kMaxSharedSlices + 2 : nullptr));
     LT_CUDA(tr, cudaGetLastError());
     tr->launches++;
     return LT_OK;

@@ -34,11 +34,10 @@ RampRing make_ring(const lt_tracker* tr) {
     return R;
 }
 
-int ensure_ramp_table(lt_tracker* tr, size_t entries) {
-    if (tr->ramp_entries >= entries) return LT_OK;
-    if (tr->ramp_table) { LT_CUDA(tr, cudaFree(tr->ramp_table)); tr->ramp_table = nullptr; tr->ramp_entries = 0; }
-    LT_CUDA(tr, cudaMalloc(&tr->ramp_table, entries * sizeof(RampEntry)));
-    tr->ramp_entries = entries;
+int ensure_ramp_table(lt_tracker* tr, size_t entries, cudaStream_t st) {
+    size_t have = tr->ramp_entries * sizeof(RampEntry);
+    LT_CUDA(tr, grow_async(&tr->ramp_table, &have, entries * sizeof(RampEntry), st));
+    if (tr->ramp_entries < entries) tr->ramp_entries = entries;
     return LT_OK;
 }
 
@@ -142,14 +141,14 @@ int lt_track_ramp(lt_tracker* tr, double* z, double* d, size_t n, unsigned long 
     if (rc || n == 0 || turns == 0) return rc;
     rc = ensure_device(tr);
     if (rc) return rc;
-    rc = ensure_sched(tr, n);
-    if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    rc = ensure_sched(tr, n, st);
+    if (rc) return rc;
     const int nsub = nsub_of(tr);
     const bool split = tr->split_drifts != 0;
     const unsigned long long chunk_max =
         std::min<unsigned long long>((unsigned long long)tr->chunk_turns, kRampChunkMax);
-    rc = ensure_ramp_table(tr, (size_t)std::min<unsigned long long>(turns, chunk_max) * nsub + 1);   // + header
+    rc = ensure_ramp_table(tr, (size_t)std::min<unsigned long long>(turns, chunk_max) * nsub + 1, st);   // + header
     if (rc) return rc;
     const PersistentPlan pl = plan_persistent(tr, n, turns, 2);
     const RampRing R = make_ring(tr);
@@ -196,12 +195,12 @@ int lt_track_ramp_per_turn(lt_tracker* tr, double* z, double* d, size_t n, unsig
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const int nsub = nsub_of(tr);
-    rc = ensure_ramp_table(tr, (size_t)turns * nsub);
+    rc = ensure_ramp_table(tr, (size_t)turns * nsub, st);
     if (rc) return rc;
     const bool moments = mo || so;
     const bool vec = aligned(z, 16) && aligned(d, 16);
     const int grid = per_turn_grid(tr, n);
-    rc = ensure_scratch(tr, grid);
+    rc = ensure_scratch(tr, grid, st);
     if (rc) return rc;
     const RampRing R = make_ring(tr);
     for (unsigned long long off = 0; off < turns; off += 1ULL << 20) {
@@ -233,8 +232,10 @@ int lt_track_ramp_per_turn(lt_tracker* tr, double* z, double* d, size_t n, unsig
                                                tr->capture_stream);
             tr->launches = before;      // capture enqueues nothing
             cudaError_t e2 = cudaStreamEndCapture(tr->capture_stream, &graph);
-            LT_CUDA(tr, e);
-            LT_CUDA(tr, e2);
+            if (e != cudaSuccess || e2 != cudaSuccess) {        // no graph is left behind on failure
+                if (graph) cudaGraphDestroy(graph);
+                LT_CUDA(tr, e != cudaSuccess ? e : e2);
+            }
             cudaError_t e3 = cudaGraphInstantiate(&tr->graph_exec, graph, 0);
             cudaGraphDestroy(graph);
             LT_CUDA(tr, e3);

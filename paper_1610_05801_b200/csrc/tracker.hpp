@@ -16,6 +16,7 @@ constexpr int kBatchTurns = 64;          // per-turn launches per finalize launc
 constexpr int kPerTurnThreads = 256;
 constexpr int kPerTurnUnroll = 2;        // double2 pairs per thread per tile
 constexpr int kMaxSlices = 1 << 20;
+constexpr int kMaxSharedSlices = 8190;   // histograms up to here are counted in shared memory (32 KB per CTA)
 constexpr int kMaxSegments = 256;        // lattice staged in shared memory by the per-turn kernel
 
 struct GraphKey {
@@ -77,6 +78,8 @@ struct lt_tracker {
     // f2: packed programme table of the current fused chunk
     double2* prog_table;
     size_t prog_entries;
+    // f4: accumulator of lt_slice_histogram (kMaxSharedSlices + 2 counters + arrival ticket), zero between calls
+    unsigned long long* hist_acc;
     // f2 with acceleration: packed sub-step entries (lt::RampEntry, 48 B each)
     void* ramp_table;
     size_t ramp_entries;
@@ -100,9 +103,26 @@ namespace lt_host {
 
 inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
 
+// Grows a tracker-owned device buffer to `need` bytes, STREAM-ORDERED on the caller's stream
+// (cudaFreeAsync + cudaMallocAsync): no device synchronisation, unlike cudaFree/cudaMalloc.  The
+// old block is released after the work already enqueued on `st`, the new one is usable by what
+// is enqueued after this call (one call in flight per tracker: include/longtrack.h).
+inline cudaError_t grow_async(void** ptr, size_t* have, size_t need, cudaStream_t st) {
+    if (*have >= need && *ptr) return cudaSuccess;
+    if (*ptr) {
+        cudaError_t e = cudaFreeAsync(*ptr, st);
+        if (e != cudaSuccess) return e;
+        *ptr = nullptr;
+        *have = 0;
+    }
+    cudaError_t e = cudaMallocAsync(ptr, need, st);
+    if (e == cudaSuccess) *have = need;
+    return e;
+}
+
 int ensure_device(lt_tracker* tr);
-int ensure_scratch(lt_tracker* tr, int grid);
-int ensure_sched(lt_tracker* tr, size_t n);
+int ensure_scratch(lt_tracker* tr, int grid, cudaStream_t st);
+int ensure_sched(lt_tracker* tr, size_t n, cudaStream_t st);
 // max_ilp: 2 where the kernel has a two-particles-per-lane instantiation, else 1
 PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns, int max_ilp = 1);
 int per_turn_grid(const lt_tracker* tr, size_t n);
