@@ -19,7 +19,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _C_FILES = ("longtrack_oracle.c", "next_oracle.c")
-_SRC = [os.path.join(_HERE, f) for f in _C_FILES + ("map.inc", "programme.inc",
+_SRC = [os.path.join(_HERE, f) for f in _C_FILES + ("map.inc", "programme.inc", "ramp.inc",
                                                      "longtrack_oracle.h", "next_oracle.h")]
 _LIB = os.path.join(_HERE, "liblongtrack_oracle.so")
 

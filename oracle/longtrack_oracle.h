@@ -28,7 +28,8 @@
  *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): exact discrete tune, determinant,
  * time reversal, bounded Hamiltonian, pendulum period vs the complete elliptic
- * integral, 40-digit hand-iterated values (tests/golden/), pure-shear / pure-kick
+ * integral, 40-digit hand-iterated values (tests/golden/; incl. phi_s = 0.3 and -0.7 for the
+ * generic kick of reading G3), pure-shear / pure-kick
  * special cases, matrix-power small-amplitude limit, 80-bit self-check, moments vs
  * numpy, membership vs brute force.  The ARITHMETIC of every function here is pinned;
  * the CHOICE of map is pinned by BASELINE.json only (the paper prints none) -- see

@@ -91,6 +91,46 @@ template <> struct Real<float> {
     static __device__ __forceinline__ float flip_by(float x, float t) { return flip(x, t); }
 };
 
+// Two fp32 particles in one 64-bit register pair.  sm_100a has packed FP32 instructions (FFMA2,
+// FADD2, FMUL2: one issue slot, two lanes' worth of arithmetic per thread), and the fp32 turn is
+// issue-bound -- the FP32 pipe takes one warp instruction per cycle, which is also all the
+// scheduler can issue, so every IMAD and loop instruction displaced an FFMA (67 % of the FP32
+// peak with scalar instructions).  Each half rounds exactly like the scalar instruction: the
+// results are the bits of Real<float>.
+struct f32x2 {
+    float2 v;
+    __host__ __device__ f32x2() {}
+    __host__ __device__ f32x2(float a) { v.x = a; v.y = a; }
+    __host__ __device__ f32x2(float a, float b) { v.x = a; v.y = b; }
+    __host__ __device__ f32x2 operator-() const { return f32x2(-v.x, -v.y); }
+};
+
+template <> struct Real<f32x2> {
+    static constexpr int NS = 5, NC = 6;
+    static __device__ __forceinline__ f32x2 magic() { return f32x2(12582912.0f); }
+    static __device__ __forceinline__ f32x2 wrap(float2 a) { f32x2 r; r.v = a; return r; }
+    static __device__ __forceinline__ f32x2 fma(f32x2 a, f32x2 b, f32x2 c) { return wrap(__ffma2_rn(a.v, b.v, c.v)); }
+    static __device__ __forceinline__ f32x2 add(f32x2 a, f32x2 b) { return wrap(__fadd2_rn(a.v, b.v)); }
+    static __device__ __forceinline__ f32x2 sub(f32x2 a, f32x2 b) { return wrap(__fadd2_rn(a.v, (-b).v)); }
+    static __device__ __forceinline__ f32x2 mul(f32x2 a, f32x2 b) { return wrap(__fmul2_rn(a.v, b.v)); }
+    static __device__ __forceinline__ f32x2 flip(f32x2 f, f32x2 t) {
+        return f32x2(Real<float>::flip(f.v.x, t.v.x), Real<float>::flip(f.v.y, t.v.y));
+    }
+    static __device__ __forceinline__ f32x2 flip_by(f32x2 x, f32x2 t) { return flip(x, t); }
+};
+
+// how many array elements of type T a register value V carries, and access to them
+template <typename T, typename V> struct Lanes {
+    static constexpr int PV = 1;
+    static __device__ __forceinline__ void set(V& v, int, T x) { v = x; }
+    static __device__ __forceinline__ T get(const V& v, int) { return v; }
+};
+template <> struct Lanes<float, f32x2> {
+    static constexpr int PV = 2;
+    static __device__ __forceinline__ void set(f32x2& v, int h, float x) { if (h) v.v.y = x; else v.v.x = x; }
+    static __device__ __forceinline__ float get(const f32x2& v, int h) { return h ? v.v.y : v.v.x; }
+};
+
 // exact reduction: returns f = v - rint(v); *t_out keeps the parity of rint(v) in its low bit
 template <typename T>
 __device__ __forceinline__ T reduce_half_periods(T v, T* t_out) {
@@ -454,15 +494,18 @@ __device__ __forceinline__ void st_release_u32(unsigned int* p, unsigned int v) 
 // back to back without a warp switch: the turn loop measures 91.5 % of the FP64 peak at 4 chains
 // per sub-partition as 2 warps x 2 chains against 87.5 % as 4 warps x 1 chain
 // (profiles/r2_fp64_pipe_probe.md).  The arithmetic per particle does not depend on ILP.
-template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ, bool PROG = false, int ILP = 1>
+// V: the register value a chain is computed in -- T itself, or f32x2 = two fp32 particles in one
+// packed value (then a lane carries 2*ILP particles and MapConsts<V> holds every constant twice).
+template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ, bool PROG = false, int ILP = 1, typename V = T>
 __global__ void __launch_bounds__(ILP == 1 ? 1024 : 512, 1)
 fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, unsigned int turns,
                         unsigned int item_turns, int first_launch, int last_launch, int dynamic,
                         unsigned long long* __restrict__ ticket, unsigned int* __restrict__ done,
-                        const __grid_constant__ MapConsts<T> P,
+                        const __grid_constant__ MapConsts<V> P,
                         const double2* __restrict__ prog = nullptr) {
     extern __shared__ __align__(16) unsigned char residency_cap[];   // sized to cap CTAs per SM; PROG: 512 B per warp of staged programme entries
-    constexpr unsigned int G = 32u * ILP;
+    typedef Lanes<T, V> L;
+    constexpr unsigned int G = 32u * ILP * L::PV;
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned long long groups = (n + G - 1) / G;
     ItemSchedule sched;
@@ -488,24 +531,30 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
             while (ld_acquire_u32(done + g) < c) __nanosleep(64);
         }
         const size_t i0 = (size_t)g * G + lane;
-        T x[ILP], dl[ILP];
+        V x[ILP], dl[ILP];
 #pragma unroll
         for (int j = 0; j < ILP; ++j) {
-            const size_t i = i0 + 32u * j;
-            x[j] = (i < n) ? __ldcg(z_arr + i) : T(0);   // L2 only: another SM may have written it
-            dl[j] = (i < n) ? __ldcg(d_arr + i) : T(0);
+#pragma unroll
+            for (int h = 0; h < L::PV; ++h) {
+                const size_t i = i0 + 32u * (j * L::PV + h);
+                L::set(x[j], h, (i < n) ? __ldcg(z_arr + i) : T(0));   // L2 only: another SM may have written it
+                L::set(dl[j], h, (i < n) ? __ldcg(d_arr + i) : T(0));
+            }
         }
         const int first = first_launch && c == 0;
         const int last = last_launch && c == nchunks - 1;
         unsigned int t_start, nt;
         sched.span(c, dynamic, &t_start, &nt);
-        advance<T, INTEG, HARM, SPLIT, ILP, FQ, PROG>(
+        advance<V, INTEG, HARM, SPLIT, ILP, FQ, PROG>(
             x, dl, nt, first, last, P, PROG ? prog + t_start : nullptr,
             PROG ? reinterpret_cast<double2*>(residency_cap) + (threadIdx.x & ~31u) : nullptr);
 #pragma unroll
         for (int j = 0; j < ILP; ++j) {
-            const size_t i = i0 + 32u * j;
-            if (i < n) { __stcg(z_arr + i, x[j]); __stcg(d_arr + i, dl[j]); }
+#pragma unroll
+            for (int h = 0; h < L::PV; ++h) {
+                const size_t i = i0 + 32u * (j * L::PV + h);
+                if (i < n) { __stcg(z_arr + i, L::get(x[j], h)); __stcg(d_arr + i, L::get(dl[j], h)); }
+            }
         }
         if (nchunks > 1) {
             __threadfence();

@@ -227,13 +227,13 @@ double loop_rate(int ilp, int w, bool fq) {
 
 }  // namespace
 namespace lt_host {
-PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns, int max_ilp) {
+PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns, int max_ilp, int pv) {
     const int sms = tr->sm_count;
     PersistentPlan best = {0, 4, 1, 512, 0, false, 1};
     double best_score = -1.0;
     for (int ilp = 1; ilp <= max_ilp; ++ilp) {
         if (max_ilp > 1 && (tr->fused_ilp == 1 || tr->fused_ilp == 2) && ilp != tr->fused_ilp) continue;
-        const unsigned long long groups = (n + 32 * ilp - 1) / (32 * ilp);
+        const unsigned long long groups = (n + 32 * ilp * pv - 1) / (32 * ilp * pv);
         const double avg = (double)groups / ((double)sms * 4);      // groups per sub-partition
         for (int w = 1; w <= 16; ++w) {
             if (w > 8 && (w & 1)) continue;                  // two CTAs per SM above 8
@@ -287,11 +287,16 @@ PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long lon
 }  // namespace lt_host
 namespace {
 
+// V = the register value of a chain: double, or f32x2 (two fp32 particles per packed value)
+template <typename T> struct ChainValue { typedef T type; };
+template <> struct ChainValue<float> { typedef f32x2 type; };
+
 template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ, int ILP>
 cudaError_t launch_persistent_ilp(T* z, T* d, size_t n, unsigned int turns, unsigned int item_turns,
                                   int first, int last, const PersistentPlan& pl, int sms,
-                                  unsigned long long* sched, const MapConsts<T>& c, cudaStream_t st) {
-    auto kern = fused_persistent_kernel<T, INTEG, HARM, SPLIT, FQ, false, ILP>;
+                                  unsigned long long* sched, const MapConsts<typename ChainValue<T>::type>& c,
+                                  cudaStream_t st) {
+    auto kern = fused_persistent_kernel<T, INTEG, HARM, SPLIT, FQ, false, ILP, typename ChainValue<T>::type>;
     // 1 CTA/SM: > half of the 227 KB; 2 CTAs/SM: > a third
     const int smem = pl.ctas_per_sm == 1 ? 120 * 1024 : 80 * 1024;
     static bool attr_set = false;                            // once per instantiation
@@ -308,7 +313,8 @@ cudaError_t launch_persistent_ilp(T* z, T* d, size_t n, unsigned int turns, unsi
 template <typename T, int INTEG, int HARM, bool SPLIT, bool FQ>
 cudaError_t launch_persistent_one(T* z, T* d, size_t n, unsigned int turns, unsigned int item_turns,
                                   int first, int last, const PersistentPlan& pl, int sms,
-                                  unsigned long long* sched, const MapConsts<T>& c, cudaStream_t st) {
+                                  unsigned long long* sched, const MapConsts<typename ChainValue<T>::type>& c,
+                                  cudaStream_t st) {
     if (pl.ilp == 2)
         return launch_persistent_ilp<T, INTEG, HARM, SPLIT, FQ, 2>(z, d, n, turns, item_turns, first, last, pl, sms, sched, c, st);
     return launch_persistent_ilp<T, INTEG, HARM, SPLIT, FQ, 1>(z, d, n, turns, item_turns, first, last, pl, sms, sched, c, st);
@@ -318,7 +324,7 @@ template <typename T, int INTEG>
 cudaError_t launch_persistent_integ(int harm, bool split, T* z, T* d, size_t n, unsigned int turns,
                                     unsigned int item_turns, int first, int last,
                                     const PersistentPlan& pl, int sms, unsigned long long* sched,
-                                    const MapConsts<T>& c, cudaStream_t st) {
+                                    const MapConsts<typename ChainValue<T>::type>& c, cudaStream_t st) {
 #define LT_PK(H, S, Q) launch_persistent_one<T, INTEG, H, S, Q>(z, d, n, turns, item_turns, first, last, pl, sms, sched, c, st)
     if (harm == 0) return LT_PK(0, true, false);
     if (harm == 1) {
@@ -341,16 +347,19 @@ int ensure_sched(lt_tracker* tr, size_t n, cudaStream_t st) {
 }  // namespace lt_host
 namespace {
 
+inline const MapConsts<double>& chain_consts(const lt_tracker* tr, double) { return tr->c64; }
+inline const MapConsts<f32x2>& chain_consts(const lt_tracker* tr, float) { return tr->c32x2; }
+
 template <typename T>
 int track_fused_persistent(lt_tracker* tr, T* z, T* d, size_t n, unsigned long long turns,
                            cudaStream_t st) {
-    const MapConsts<T>& c = *reinterpret_cast<const MapConsts<T>*>(
-        sizeof(T) == 8 ? (const void*)&tr->c64 : (const void*)&tr->c32);
+    const MapConsts<typename ChainValue<T>::type>& c = chain_consts(tr, T());
+    constexpr int kPV = sizeof(typename ChainValue<T>::type) / sizeof(T);   // particles per chain value
     const bool split = tr->split_drifts != 0 || tr->harm == 0;
     int rc = ensure_sched(tr, n, st);
     if (rc) return rc;
     unsigned long long done = 0;
-    PersistentPlan pl = plan_persistent(tr, n, turns, 2);
+    PersistentPlan pl = plan_persistent(tr, n, turns, 2, kPV);
     while (done < turns) {
         unsigned long long chunk = std::min<unsigned long long>(turns - done, (unsigned long long)tr->chunk_turns);
         const int first = done == 0, last = done + chunk == turns;
@@ -375,7 +384,7 @@ int track_fused_persistent(lt_tracker* tr, T* z, T* d, size_t n, unsigned long l
     }
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
-    tr->last_ilp = pl.ilp;
+    tr->last_ilp = pl.ilp * kPV;
     tr->last_mode = pl.dynamic ? 3 : 2;
     tr->last_item_turns = pl.dynamic ? pl.item_turns : 0;
     return LT_OK;
@@ -636,6 +645,12 @@ int lt_create(const lt_params* p, lt_tracker** out) {
     tr->g = g;
     fill_consts<double>(p, &tr->c64);
     fill_consts<float>(p, &tr->c32);
+    {   // every fp32 constant twice: the packed (two particles per value) form of the same numbers
+        static_assert(sizeof(MapConsts<f32x2>) == 2 * sizeof(MapConsts<float>), "packed constants");
+        const float* src = reinterpret_cast<const float*>(&tr->c32);
+        float* dst = reinterpret_cast<float*>(&tr->c32x2);
+        for (size_t k = 0; k < sizeof(MapConsts<float>) / sizeof(float); ++k) { dst[2 * k] = src[k]; dst[2 * k + 1] = src[k]; }
+    }
     tr->harm = (p->phi_s != 0.0) ? 0 : (p->ratio2 != 0.0 ? 2 : 1);
     tr->split_drifts = 0;
     tr->chunk_turns = 1LL << 22;

@@ -52,6 +52,7 @@ struct lt_tracker {
     lt_derived_t g;
     lt::MapConsts<double> c64;
     lt::MapConsts<float> c32;
+    lt::MapConsts<lt::f32x2> c32x2;   // c32 with every constant twice (packed fp32 pairs)
     int harm;                 // 0 generic (phi_s != 0), 1 single, 2 double harmonic
     // options
     long long split_drifts, chunk_turns, fused_ilp, fused_block, per_turn_graph,
@@ -124,7 +125,8 @@ int ensure_device(lt_tracker* tr);
 int ensure_scratch(lt_tracker* tr, int grid, cudaStream_t st);
 int ensure_sched(lt_tracker* tr, size_t n, cudaStream_t st);
 // max_ilp: 2 where the kernel has a two-particles-per-lane instantiation, else 1
-PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns, int max_ilp = 1);
+// pv: particles per chain value (2 for packed fp32 pairs)
+PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns, int max_ilp = 1, int pv = 1);
 int per_turn_grid(const lt_tracker* tr, size_t n);
 // the BASELINE path's fused / per-turn entry points, for calls that compose with them
 int track_fused_f64(lt_tracker* tr, double* z, double* d, size_t n, unsigned long long turns,

@@ -191,8 +191,10 @@ def test_product_path_never_touches_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
                 assert "longtrack_oracle" not in text and "lto_" not in text, f
-    for f in ("longtrack_oracle.c", "map.inc", "longtrack_oracle.h", "__init__.py", "next_oracle.c",
-              "next_oracle.h", "programme.inc"):
+    oracle_files = sorted(f for f in os.listdir(os.path.join(ROOT, "oracle"))
+                          if f.endswith((".c", ".h", ".inc", ".py")))
+    assert {"longtrack_oracle.c", "map.inc", "programme.inc", "ramp.inc", "next_oracle.c"} <= set(oracle_files)
+    for f in oracle_files:
         text = open(os.path.join(ROOT, "oracle", f)).read()
         assert "paper_1610_05801_b200" not in text.replace(
             "paper_1610_05801_b200/csrc/, include/longtrack.h", "").replace(
