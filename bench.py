@@ -369,10 +369,12 @@ def bench_f1(cx: Ctx) -> dict:
 
 
 # ----------------------------------------------------------------------------- FP64 pipe probe
-def bench_probe(cx: Ctx) -> dict:
+def bench_probe(cx: Ctx, table: bool = False) -> dict:
     """What the FP64 pipe of this device issues (lt_probe_pipe, clock64-based): FP64
     warp-instructions per cycle and sub-partition; the nominal peak behind roofline.peak is 0.5
-    (16 FP64 lanes per sub-partition, 64 per SM)."""
+    (16 FP64 lanes per sub-partition, 64 per SM).  table=True (`--only probe`) adds the rate of
+    the turn loop for every (particles per lane, warps per sub-partition, sign-flip place): the
+    planner's loop_rate table in csrc/longtrack.cu."""
     lt = cx.lt
     out = {}
     with cx.clock() as clk:
@@ -387,7 +389,57 @@ def bench_probe(cx: Ctx) -> dict:
             rate, mhz = lt.probe_pipe(kind, SMS, threads, chains, 20000 // chains)
             out[name] = round(rate, 4)
             out["sm_mhz_under_fp64_load"] = round(mhz)
+        if table:
+            tab = {}
+            for kind, name in ((11, "flip_on_f"), (10, "flip_on_q"), (12, "no_flip")):
+                for chains in (1, 2, 4):
+                    tab["%s ilp%d W=1..8" % (name, chains)] = [
+                        round(lt.probe_pipe(kind, SMS, 128 * w, chains, 8000 // chains)[0], 4)
+                        for w in range(1, 9)]
+            out["turn_loop_table"] = tab
     out["unit"] = "FP64 warp-instr/cycle/sub-partition (nominal peak 0.5)"
+    out["clocks"] = clk.summary(short=True)
+    return out
+
+
+# ----------------------------------------------------------------------------- launch-shape sweep
+def bench_shapes(cx: Ctx) -> dict:
+    """`--only shapes`: the planner against forced launch shapes of the fused kernel (particles per
+    lane, warps per sub-partition, sign-flip place, item length) at the configs[1] size and at
+    10^6 particles x 10^4 turns -- what profiles/r2_fused_shapes.md tabulates."""
+    lt, wl = cx.lt, cx.wl
+    out = {}
+    with cx.clock() as clk:
+        for n, turns, cfg in ((100_000, 70_000, wl.CONFIGS[1]), (1_000_000, 10_000, wl.CONFIGS[2])):
+            z0, d0 = wl.make_bunch(cfg, n=n)
+            z, d = cx.dev(z0), cx.dev(d0)
+            cases = [("planner", {})]
+            for ilp, w, fq in ((2, 1, 0), (2, 2, 0), (2, 2, 1), (2, 3, 0), (2, 4, 0), (2, 4, 1),
+                               (1, 4, 1), (1, 5, 0), (1, 5, 1), (1, 6, 1), (1, 8, 0), (1, 8, 1)):
+                for item in ((512, 2048, 8192) if (ilp, w, fq) in ((2, 2, 0), (2, 4, 0), (1, 5, 1)) else (2048,)):
+                    cases.append(("ilp%d W%d %s item%d" % (ilp, w, "q" if fq else "f", item),
+                                  {lt.OPT_FUSED_MODE: 3, lt.OPT_FUSED_ILP: ilp, lt.OPT_WARPS_PER_SMSP: w,
+                                   lt.OPT_FLIP_ON_Q: fq, lt.OPT_ITEM_TURNS: item}))
+            for w in (4, 8):
+                cases.append(("static ilp2 W%d" % w, {lt.OPT_FUSED_MODE: 2, lt.OPT_FUSED_ILP: 2,
+                                                        lt.OPT_WARPS_PER_SMSP: min(w, 4)}))
+                cases.append(("static ilp1 W%d" % w, {lt.OPT_FUSED_MODE: 2, lt.OPT_FUSED_ILP: 1,
+                                                        lt.OPT_WARPS_PER_SMSP: w}))
+            cases.append(("plain kernel block64 ilp2", {lt.OPT_FUSED_MODE: 1, lt.OPT_FUSED_ILP: 2,
+                                                        lt.OPT_FUSED_BLOCK: 64}))
+            rows = {}
+            for label, opts in cases:
+                tr = lt.Tracker(wl.RING, "leapfrog")
+                for k, v in opts.items():
+                    tr.set_option(k, v)
+                sec = cx.timed(lambda: tr.track_fused(z, d, n, turns, cx.sp), 3, flush=False)
+                rows[label] = {"ms": round(1e3 * sec, 3),
+                               "frac": round(FP64_INSTR_PER_PT * n * turns / sec / 1e9 / cx.peak_fp64, 4),
+                               "block": tr.get_stat(lt.STAT_LAST_BLOCK), "ilp": tr.get_stat(lt.STAT_LAST_ILP),
+                               "item": tr.get_stat(lt.STAT_LAST_ITEM_TURNS)}
+                del tr
+            out["n=%d turns=%d" % (n, turns)] = rows
+            del z, d
     out["clocks"] = clk.summary(short=True)
     return out
 
@@ -549,7 +601,7 @@ def bench_per_turn_sharded(cx: Ctx) -> dict:
     import numpy as np
     lt, wl, torch = cx.lt, cx.wl, cx.torch
     c3 = wl.CONFIGS[3]
-    n, turns = 1_000_003, 256                      # odd shards; the second starts 8-byte aligned
+    n, turns = 1_000_001, 256                      # odd first shard: the second starts 8-byte aligned
     z0, d0 = wl.make_bunch(c3, n=n)
     nshard = cx.world if cx.world > 1 else 2
     mine = [cx.rank] if cx.world > 1 else [0, 1]
@@ -600,7 +652,8 @@ def run_cuda(args) -> None:
 
     if args.only:                                        # profiling aid: one leg, printed alone
         leg = {"per_turn": bench_per_turn, "configs": bench_configs, "f1": bench_f1,
-               "next": bench_next, "probe": bench_probe, "sharded": bench_per_turn_sharded}.get(args.only)
+               "next": bench_next, "probe": lambda c: bench_probe(c, table=True), "shapes": bench_shapes,
+               "sharded": bench_per_turn_sharded}.get(args.only)
         if leg is not None:
             res = leg(cx)
             if rank == 0:
@@ -745,7 +798,7 @@ def main():
     ap.add_argument("--skip-cpu", action="store_true")
     ap.add_argument("--skip-next", action="store_true")
     ap.add_argument("--only", default=None,
-                    choices=["headline", "per_turn", "sharded", "configs", "f1", "next", "probe"],
+                    choices=["headline", "per_turn", "sharded", "configs", "f1", "next", "probe", "shapes"],
                     help="run one leg alone (for ncu captures and sweeps)")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -157,9 +157,10 @@ __device__ __forceinline__ T horner(const T (&c)[N], T s) {
 //   HARM = 2: F = A [sin(pi v) + r sin(2 pi v)] = A sin(pi v) (1 + 2 r cos(pi v))   (configs[4])
 //   HARM = 0: generic, phi_s != 0:  A [sin(phi_s + pi v) - sin(phi_s) + r sin(2 pi v)]   (G3)
 // ------------------------------------------------------------------------------------------
-// FQ selects WHERE the sign (-1)^n is applied: to f (off the critical path, best below ~5
-// resident warps per sub-partition) or to the polynomial value q (one dependent integer op
-// later, but it measured 3-4 % faster once the FP64 pipe is saturated; profiles/r1_fused_sweep.md).
+// FQ selects WHERE the sign (-1)^n is applied: to f (beside the Horner chain: wins with two
+// particles per lane at every warp count) or to the polynomial value q (one dependent integer
+// op later, but faster with ONE particle per lane from 5 warps per sub-partition on;
+// profiles/r2_fp64_pipe_probe.md).  Same bits either way.
 // PROG (RF programme; G28): the kick of this turn is
 //     a * A [ sin(phi_s + pi (v + p)) - sin(phi_s) + r sin(2 pi (v + p)) ],
 // a = voltage scale, p = phase offset in half periods.  PROG = 1: add p here (fast path, the
@@ -341,8 +342,8 @@ __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int 
                 if (INTEG != kEulerCromer) x[j] = R::fma(-P.drift_lead, dl[j], x[j]);
             }
         }
-        // every non-FP64 instruction costs about two issue cycles next to the saturated FP64
-        // pipe (profiles/r1_fused_sweep.md): unroll deep enough that the loop counter disappears
+        // every non-FP64 instruction costs issue capacity next to the saturated FP64 pipe
+        // (profiles/r2_fp64_pipe_probe.md): unroll deep enough that the loop counter disappears
         constexpr int kUnroll = (INTEG == kRuth4 || HARM != 1 || ILP > 2) ? 4 : LT_TURN_UNROLL / ILP;
 #pragma unroll kUnroll
         for (unsigned int t = 1; t < turns; ++t) {
@@ -445,7 +446,7 @@ __global__ void fused_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_
 // (dynamic scheduling): full items first, then the last item..2*item turns are halved again and
 // again down to kMinTaper turns, so that the warps which find the ticket queue empty wait for a
 // short item, not a long one (an untapered tail cost 1.7 % at 10^5 particles,
-// profiles/r2_item_sweep.md).  Chunk boundaries never change the arithmetic (G16).
+// profiles/r2_fused_shapes.md).  Chunk boundaries never change the arithmetic (G16).
 constexpr unsigned int kMinTaper = 64;
 struct ItemSchedule {
     unsigned int turns, item, nfull, nchunks;

@@ -274,7 +274,7 @@ PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long lon
         // an item switch costs a warp about 3 us (ticket, progress word, state load; store, fence,
         // release), during which its sub-partition runs at half rate when it holds two warps: long
         // items (2048 turns = 120 us) amortise that, and the tapered tail of the schedule
-        // (ItemSchedule) keeps the last round short all the same (profiles/r2_item_sweep.md)
+        // (ItemSchedule) keeps the last round short all the same (profiles/r2_fused_shapes.md)
         unsigned long long it = tr->item_turns > 0
                                     ? (unsigned long long)tr->item_turns
                                     : std::min<unsigned long long>(2048, std::max<unsigned long long>(128, turns / 8));

@@ -95,8 +95,9 @@ def test_split_drift_mode_is_bit_identical_across_calls_and_modes(integrator, ra
 @pytest.mark.parametrize("integrator", INTEGRATORS)
 @pytest.mark.parametrize("ratio2", [0.0, 0.5])
 def test_dynamic_scheduling_is_bit_identical_to_the_plain_kernel(integrator, ratio2):
-    """The on-device chunk scheduler (work items = 32 particles x item_turns) must not change a
-    single bit, merged or split drifts, whatever the item length."""
+    """The on-device chunk scheduler (work items = 32 or 64 particles x item_turns, tapered at the
+    end of a launch) must not change a single bit, merged or split drifts, whatever the item
+    length and the number of particles per lane."""
     tr, _ = both(integrator, ratio2)
     z0, d0 = wl.make_bunch(wl.CONFIGS[4], n=150_001)
     for split in (0, 1):
@@ -104,10 +105,12 @@ def test_dynamic_scheduling_is_bit_identical_to_the_plain_kernel(integrator, rat
         tr.set_option(lt.OPT_FUSED_MODE, lt.FUSED_PLAIN)
         ref = gpu_track(tr, z0, d0, 777)
         tr.set_option(lt.OPT_FUSED_MODE, lt.FUSED_PERSISTENT_DYNAMIC)
-        for item in (0, 50, 776):
-            tr.set_option(lt.OPT_ITEM_TURNS, item)
-            out = gpu_track(tr, z0, d0, 777)
-            assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1]), (split, item)
+        for ilp in (1, 2, 0):                           # one / two particles per lane / planner
+            tr.set_option(lt.OPT_FUSED_ILP, ilp)
+            for item in (0, 50, 200, 776):              # 200: full items + a tapered tail of 377
+                tr.set_option(lt.OPT_ITEM_TURNS, item)
+                out = gpu_track(tr, z0, d0, 777)
+                assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1]), (split, ilp, item)
         tr.set_option(lt.OPT_CHUNK_TURNS, 300)          # several launches, each with its own items
         out = gpu_track(tr, z0, d0, 777)
         assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1])
@@ -141,17 +144,22 @@ def test_ragged_sizes_all_layouts(n):
             tr.set_option(lt.OPT_FUSED_BLOCK, block)
             zg, dg = gpu_track(tr, z0, d0, 100)
             assert np.array_equal(zg, zr) and np.array_equal(dg, dr), (ilp, block)
-    for mode, w, item, fq in ((lt.FUSED_PERSISTENT_STATIC, 0, 0, 0), (lt.FUSED_PERSISTENT_STATIC, 1, 0, 1),
-                              (lt.FUSED_PERSISTENT_STATIC, 16, 0, -1), (lt.FUSED_PERSISTENT_DYNAMIC, 0, 0, -1),
-                              (lt.FUSED_PERSISTENT_DYNAMIC, 5, 7, 0), (lt.FUSED_PERSISTENT_DYNAMIC, 8, 33, 1),
-                              (lt.FUSED_PERSISTENT_DYNAMIC, 2, 1, 1), (lt.FUSED_PERSISTENT_DYNAMIC, 12, 100, 0)):
-        tr.set_option(lt.OPT_FUSED_MODE, mode)
-        tr.set_option(lt.OPT_WARPS_PER_SMSP, w)
-        tr.set_option(lt.OPT_ITEM_TURNS, item)
-        tr.set_option(lt.OPT_FLIP_ON_Q, fq)
-        zg, dg = gpu_track(tr, z0, d0, 100)
-        assert np.array_equal(zg, zr) and np.array_equal(dg, dr), (mode, w, item, fq)
-        assert tr.get_stat(lt.STAT_LAST_MODE) == mode
+    for ilp in (1, 2):                                        # particles per lane of the persistent kernel
+        tr.set_option(lt.OPT_FUSED_ILP, ilp)
+        for mode, w, item, fq in ((lt.FUSED_PERSISTENT_STATIC, 0, 0, 0), (lt.FUSED_PERSISTENT_STATIC, 1, 0, 1),
+                                  (lt.FUSED_PERSISTENT_STATIC, 16 if ilp == 1 else 4, 0, -1),
+                                  (lt.FUSED_PERSISTENT_DYNAMIC, 0, 0, -1),
+                                  (lt.FUSED_PERSISTENT_DYNAMIC, 5 if ilp == 1 else 3, 7, 0),
+                                  (lt.FUSED_PERSISTENT_DYNAMIC, 8 if ilp == 1 else 4, 33, 1),
+                                  (lt.FUSED_PERSISTENT_DYNAMIC, 2, 1, 1),
+                                  (lt.FUSED_PERSISTENT_DYNAMIC, 12 if ilp == 1 else 1, 100, 0)):
+            tr.set_option(lt.OPT_FUSED_MODE, mode)
+            tr.set_option(lt.OPT_WARPS_PER_SMSP, w)
+            tr.set_option(lt.OPT_ITEM_TURNS, item)
+            tr.set_option(lt.OPT_FLIP_ON_Q, fq)
+            zg, dg = gpu_track(tr, z0, d0, 100)
+            assert np.array_equal(zg, zr) and np.array_equal(dg, dr), (ilp, mode, w, item, fq)
+            assert tr.get_stat(lt.STAT_LAST_MODE) == mode and tr.get_stat(lt.STAT_LAST_ILP) == ilp
     zg, dg, mg = gpu_track(tr, z0, d0, 100, "per_turn", want_moments=True)
     assert_particle_gate(p, z0, d0, zg, dg, zo, do, sd, gate=1e-10)
     mo = oracle.moments_of(p, zo, do)
@@ -378,6 +386,47 @@ def test_cfg3_full_size_per_turn_moments():
     last = oracle.moments_of(p, zg, dg)
     assert_moments_close(mg[-1:], {k: [v] for k, v in last.items()})
     assert int(mg["n_in_bucket"][-1]) == last["n_in_bucket"]
+
+
+def test_sharded_per_turn_path_on_one_gpu():
+    """SURVEY.md sec. 8(e) on ONE device: a configs[3]-shaped bunch of 1 000 001 particles is split
+    with workloads.shard_range into two contiguous ranges of ONE device array -- the first of odd
+    size, so that the second starts 8-byte aligned (scalar path) -- and tracked by two trackers on two
+    streams with raw sums; the two lt_sums[turns] are added on the host (what the all-reduce does),
+    lt_moments_from_sums finalises.  Must equal the unsharded GPU run (state: same bits; moments:
+    1e-13; counts exact) and the oracle (1e-6; counts exact).  Unmeasured on multi-GPU hardware."""
+    tr, p = both()
+    n, turns = 1_000_001, 200                            # 3 graph replays of 64 + a tail of 8
+    z0, d0 = wl.make_bunch(wl.CONFIGS[3], n=n)
+    zu, du, mu = gpu_track(tr, z0, d0, turns, "per_turn", want_moments=True)
+    zs, ds = dev(z0), dev(d0)
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    trackers = [lt.Tracker(wl.RING, "leapfrog"), lt.Tracker(wl.RING, "leapfrog")]
+    sums = [torch.zeros(turns * lt.SUMS_DTYPE.itemsize, dtype=torch.uint8, device="cuda") for _ in range(2)]
+    torch.cuda.synchronize()
+    for k in range(2):
+        lo, hi = wl.shard_range(n, k, 2)
+        zk, dk = zs[lo:hi], ds[lo:hi]
+        if k == 0:
+            assert (hi - lo) % 2 == 1 and zk.data_ptr() % 16 == 0
+        else:
+            assert zk.data_ptr() % 16 == 8
+        trackers[k].track_per_turn(zk, dk, hi - lo, turns, None, sums[k], streams[k].cuda_stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(zs.cpu().numpy(), zu) and np.array_equal(ds.cpu().numpy(), du)
+    parts = [s.cpu().numpy().view(lt.SUMS_DTYPE) for s in sums]
+    total = np.zeros(turns, dtype=lt.SUMS_DTYPE)
+    for name in lt.SUMS_DTYPE.names:
+        total[name] = parts[0][name] + parts[1][name]    # the SUM all-reduce
+    assert np.all(total["n"] == n)
+    ms = lt.moments_from_sums(total)
+    assert np.array_equal(ms["n_in_bucket"], mu["n_in_bucket"])
+    for name in ("rms_z", "rms_d"):
+        assert np.max(np.abs(ms[name] / mu[name] - 1)) <= 1e-13, name
+    assert np.max(np.abs(ms["mean_z"] - mu["mean_z"])) <= 1e-13 * mu["rms_z"].max()
+    _, _, mo = oracle.track_moments(p, z0, d0, turns)
+    assert_moments_close(ms, mo)
+    assert np.array_equal(ms["n_in_bucket"], mo["n_in_bucket"])
 
 
 def test_per_turn_moments_medium_all_turns_graph_and_plain():

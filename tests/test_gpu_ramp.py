@@ -123,6 +123,33 @@ def test_ramp_call_lengths_around_the_staging_block(turns):
             assert_close(p, zg, dg, zo, do, gate=1e-11)
 
 
+@pytest.mark.parametrize("integrator", ["leapfrog", "ruth4"])
+def test_ramp_every_launch_shape_returns_the_same_bits(integrator):
+    """Warps per sub-partition 1 .. 16 (two CTAs per SM above 8: 32 warps x 3072 B of staging in
+    each), one and two particles per lane, static and dynamic scheduling: same bits as the
+    planner's launch, merged and split drifts."""
+    tr, _ = both(integrator)
+    n, turns = 40_003, 333
+    z0, d0 = wl.gaussian_bunch(n, 0.08, 91)
+    p0c, a, psi = wl.energy_ramp(turns, 26e9, 26.08e9)
+    for split in (0, 1):
+        tr.set_option(lt.OPT_SPLIT_DRIFTS, split)
+        for opt in (lt.OPT_FUSED_MODE, lt.OPT_FUSED_ILP, lt.OPT_WARPS_PER_SMSP, lt.OPT_ITEM_TURNS):
+            tr.set_option(opt, 0)
+        ref = gpu_ramp(tr, z0, d0, p0c, a, psi)
+        for mode, ilp, w, item in ((lt.FUSED_PERSISTENT_DYNAMIC, 1, 14, 40), (lt.FUSED_PERSISTENT_DYNAMIC, 1, 16, 0),
+                                   (lt.FUSED_PERSISTENT_STATIC, 1, 16, 0), (lt.FUSED_PERSISTENT_DYNAMIC, 1, 8, 100),
+                                   (lt.FUSED_PERSISTENT_DYNAMIC, 2, 1, 64), (lt.FUSED_PERSISTENT_DYNAMIC, 2, 4, 0),
+                                   (lt.FUSED_PERSISTENT_STATIC, 2, 3, 0), (lt.FUSED_PERSISTENT_DYNAMIC, 1, 3, 7)):
+            tr.set_option(lt.OPT_FUSED_MODE, mode)
+            tr.set_option(lt.OPT_FUSED_ILP, ilp)
+            tr.set_option(lt.OPT_WARPS_PER_SMSP, w)
+            tr.set_option(lt.OPT_ITEM_TURNS, item)
+            out = gpu_ramp(tr, z0, d0, p0c, a, psi)
+            assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1]), (split, mode, ilp, w, item)
+            assert tr.get_stat(lt.STAT_LAST_ILP) == ilp
+
+
 def test_ramp_per_turn_moments_every_turn_graph_and_plain():
     tr, p = both()
     z0, d0 = wl.gaussian_bunch(20_001, 0.1, 44)
