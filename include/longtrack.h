@@ -35,8 +35,17 @@
  *     required; 16-byte alignment enables the vector path (otherwise a scalar path runs).
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
  *     calls only ENQUEUE work on that stream and return; nothing synchronises the device.
- *     Results are valid once the caller has synchronised the stream.  The *_host calls are
- *     the exception: they copy, run and copy back, and return after the data is on the host.
+ *     Results are valid once the caller has synchronised the stream.  The *_host calls and the
+ *     lt_probe_* calls are the exception: they run to completion before they return.
+ *     The tracker's scratch is grown STREAM-ORDERED on the caller's stream (cudaMallocAsync /
+ *     cudaFreeAsync): a call that needs more scratch than any before it (a larger n, a longer
+ *     table) allocates without a device synchronisation, but it must not be issued while the
+ *     stream is being CAPTURED into a CUDA graph by the caller -- run the call once uncaptured
+ *     at the largest size first.
+ *   - If a device call returns LT_E_CUDA part-way through a fused call that needed several
+ *     launches (LT_OPT_CHUNK_TURNS smaller than `turns`), the arrays hold an intermediate state:
+ *     in the default merged-drift mode z is then the RF phase in half periods, mid-drift, NOT
+ *     metres.  Treat z/delta as lost after LT_E_CUDA.
  *   - Return value: 0 = LT_OK, negative = error (below).  The library never throws, aborts
  *     or prints.  n == 0 or turns == 0 is LT_OK and a no-op.
  *   - One tracker may have ONE call in flight at a time (the scratch is per tracker); use
@@ -125,7 +134,9 @@ enum {
                                   per-turn kernel and to any chunking by the caller.       */
     LT_OPT_CHUNK_TURNS    = 2, /* turns per fused kernel launch (default 2^22); the result
                                   of one call does not depend on it     */
-    LT_OPT_FUSED_ILP      = 3, /* particles per thread in fused mode: 0 = planner decides  */
+    LT_OPT_FUSED_ILP      = 3, /* particles per lane in fused mode: 0 = planner decides; 1, 2 for
+                                  the persistent kernels (fp32: PAIRS of particles per lane, the
+                                  arithmetic is packed two to a value), 1, 2, 4 for the plain one  */
     LT_OPT_FUSED_BLOCK    = 4, /* threads per block in fused mode: 0 = planner decides     */
     LT_OPT_PER_TURN_GRAPH = 5, /* 1 (default): per-turn launches are replayed from a CUDA
                                   graph in batches; 0: plain stream launches               */
@@ -136,9 +147,11 @@ enum {
                                   dynamic form; 1: plain one-thread-per-particle kernel
                                   (LT_OPT_FUSED_ILP / _BLOCK apply); 3: force dynamic        */
     LT_OPT_ITEM_TURNS     = 9, /* turns per work item of the dynamic persistent kernel
-                                  (0 = planner: 256..1024); results do not depend on it            */
+                                  (0 = planner: 128..2048; the last items of a launch are halved
+                                  again and again); results do not depend on it                    */
     LT_OPT_WARPS_PER_SMSP = 10,/* resident warps per SM sub-partition of the persistent kernel
-                                  (0 = planner; 1..8, or even values up to 16)              */
+                                  (0 = planner; 1..8, or even values up to 16; with two particles
+                                  per lane at most 4)                                               */
     LT_OPT_FLIP_ON_Q      = 11 /* where the sign of the reduced sine is applied: -1 planner,
                                   0 on the argument, 1 on the polynomial; same bits either way */
 };
@@ -148,7 +161,7 @@ enum {
     LT_STAT_KERNEL_LAUNCHES = 1, /* kernels launched by this tracker since creation        */
     LT_STAT_LAST_GRID       = 2, /* grid / block / ilp of the last fused launch            */
     LT_STAT_LAST_BLOCK      = 3,
-    LT_STAT_LAST_ILP        = 4,
+    LT_STAT_LAST_ILP        = 4, /* particles per lane of the last fused launch             */
     LT_STAT_SM_COUNT        = 5,
     LT_STAT_LAST_MODE       = 6, /* 1 plain, 2 persistent static, 3 persistent dynamic          */
     LT_STAT_LAST_ITEM_TURNS = 7
@@ -192,7 +205,14 @@ int lt_track_per_turn_f32(lt_tracker *tr, float *z_dev, float *delta_dev, size_t
 /* -- observables of the current state ---------------------------------------------------- */
 
 /* Bucket membership (BASELINE.json:north_star "bucket-membership counts (exact)";
- * DESIGN.md G15): count_dev[0] = #{ i : |z_i| < z_max  and  H(z_i, delta_i) < H_sep }. */
+ * DESIGN.md G15): count_dev[0] = #{ i : |z_i| < z_max  and  H(z_i, delta_i) < H_sep } with
+ *     H(z, delta) = eta C delta^2 / 2 + (A R / h) [(1 - cos kappa z) + (r/2)(1 - cos 2 kappa z)],
+ *     z_max = pi R / h,  H_sep = 2 A R / h
+ * -- the STATIONARY bucket of phi_s = 0 with -1/2 <= r <= 1/2, which is every BASELINE config.
+ * The same predicate fills n_in_bucket of lt_moments / lt_sums everywhere.  Outside that range
+ * it is still evaluated as written but is no longer "the bucket": for phi_s != 0 the bucket is
+ * asymmetric and smaller, for |r| > 1/2 the potential has extra extrema inside +-z_max; with
+ * A = 0 (no RF) H_sep = 0 and the count is 0. */
 int lt_bucket_count(lt_tracker *tr, const double *z_dev, const double *delta_dev, size_t n,
                     unsigned long long *count_dev, void *stream);
 int lt_bucket_count_f32(lt_tracker *tr, const float *z_dev, const float *delta_dev, size_t n,
@@ -254,10 +274,11 @@ int lt_track_programme_per_turn(lt_tracker *tr, double *z_dev, double *delta_dev
  * pb -> pb + x1 D -> (that) + x0 D -> pa.  A particle at z = 0, delta = 0 stays on the reference iff
  * a_t A(pb) sin(psi_t) = D/pb: the caller programmes the synchronous phase through psi_t, so
  * lt_params.phi_s must be 0 here (else LT_E_PARAM).  The tracker's own parameters are not changed
- * by the call.  lt_track_ramp: fused multi-turn mode (17 FP64 instructions per sub-step);
+ * by the call.  lt_track_ramp: fused multi-turn mode (16 FP64 instructions per sub-step);
  * lt_track_ramp_per_turn: per-turn mode with the outputs of lt_track_per_turn (n_in_bucket is the
- * stationary-bucket predicate of lt_params, whatever the ramp does).  The tables are read while
- * the call's work runs: keep them unchanged until the stream has been synchronised. */
+ * stationary-bucket predicate of lt_params, whatever the ramp does; at most 2^26 turns per call,
+ * else LT_E_PARAM: the whole call's table is packed at once).  The tables are read while the
+ * call's work runs: keep them unchanged until the stream has been synchronised. */
 int lt_track_ramp(lt_tracker *tr, double *z_dev, double *delta_dev, size_t n,
                   unsigned long long turns, const double *p0c_dev, const double *volt_scale_dev,
                   const double *phase_off_dev, void *stream);
