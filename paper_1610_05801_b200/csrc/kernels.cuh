@@ -113,8 +113,14 @@ template <> struct Real<f32x2> {
     static __device__ __forceinline__ f32x2 add(f32x2 a, f32x2 b) { return wrap(__fadd2_rn(a.v, b.v)); }
     static __device__ __forceinline__ f32x2 sub(f32x2 a, f32x2 b) { return wrap(__fadd2_rn(a.v, (-b).v)); }
     static __device__ __forceinline__ f32x2 mul(f32x2 a, f32x2 b) { return wrap(__fmul2_rn(a.v, b.v)); }
+    // With packed arithmetic the FMA pipe is the bound (two cycles per FFMA2) and issue slots are
+    // free, so the sign flip leaves that pipe: funnel shift + XOR on the ALU pipe instead of the
+    // IMAD of the scalar kernels (an IMAD occupies the FMA pipe; profiles/r2_ncu_summary.md).
+    static __device__ __forceinline__ float flip1(float f, float t) {
+        return __uint_as_float(__float_as_uint(f) ^ __funnelshift_l(0u, __float_as_uint(t), 31));
+    }
     static __device__ __forceinline__ f32x2 flip(f32x2 f, f32x2 t) {
-        return f32x2(Real<float>::flip(f.v.x, t.v.x), Real<float>::flip(f.v.y, t.v.y));
+        return f32x2(flip1(f.v.x, t.v.x), flip1(f.v.y, t.v.y));
     }
     static __device__ __forceinline__ f32x2 flip_by(f32x2 x, f32x2 t) { return flip(x, t); }
 };
