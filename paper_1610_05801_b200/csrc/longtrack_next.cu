@@ -342,8 +342,12 @@ cudaError_t launch_transverse_one(double* x, double* xp, double* y, double* yp, 
                                   const PersistentPlan& pl, const lt_tracker* tr, cudaStream_t st) {
     auto kern = transverse_persistent_kernel<NSEG, LONGI, ILP>;
     const int smem = residency_smem(pl);                 // >= the lattice (256 x 128 B)
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
+    static bool attr_set = false;                        // once per instantiation
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
     kern<<<tr->sm_count * pl.ctas_per_sm, pl.threads, smem, st>>>(
         x, xp, y, yp, z, d, n, turns, item_turns, first, last, pl.dynamic, tr->sched,
         reinterpret_cast<unsigned int*>(tr->sched + 1), tr->lattice_dev, tr->n_seg, tr->c64);
