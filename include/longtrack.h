@@ -329,6 +329,19 @@ int lt_track_transverse_per_turn(lt_tracker *tr, double *x_dev, double *xp_dev, 
                                  double *yp_dev, double *z_dev, double *delta_dev, size_t n,
                                  unsigned long long turns, void *stream);
 
+/* -- introspection of the host logic (no GPU needed; what the CPU tests call) ---------------
+ * lt_plan_fused: the launch shape lt_track_fused would pick for n particles and `turns` turns on
+ * a device with sm_count SMs (options of the tracker apply): plan[0] = 1 dynamic work queue / 0
+ * static slots, plan[1] = warps per sub-partition, plan[2] = CTAs per SM, plan[3] = threads per
+ * CTA, plan[4] = turns per work item (0 = all), plan[5] = sign flip on q, plan[6] = particles per
+ * lane (fp32: pairs count double).
+ * lt_item_schedule: the tapered work-item schedule of a launch: number of
+ * chunks, and first turn / length of chunk c (c >= *nchunks: LT_E_PARAM). */
+int lt_plan_fused(const lt_tracker *tr, size_t n, unsigned long long turns, int sm_count, int fp32,
+                  long long plan[7]);
+int lt_item_schedule(unsigned int turns, unsigned int item_turns, int taper, unsigned int c,
+                     unsigned int *nchunks, unsigned int *start, unsigned int *len);
+
 /* -- roofline probes (measurement only, not on the hot path) ------------------------------
  * Runs a dependent-chain DFMA kernel (`chains` independent chains per thread, `iters` FMAs
  * per chain) and returns achieved FP64 lane-instructions per second in *rate. Synchronises. */

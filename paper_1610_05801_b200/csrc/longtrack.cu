@@ -845,6 +845,36 @@ int lt_track_fused_host(lt_tracker* tr, double* z_host, double* delta_host, size
     return LT_OK;
 }
 
+int lt_plan_fused(const lt_tracker* tr, size_t n, unsigned long long turns, int sm_count, int fp32,
+                  long long plan[7]) {
+    if (!tr || !plan) return LT_E_NULL;
+    if (sm_count < 1 || n == 0 || turns == 0) return LT_E_PARAM;
+    lt_tracker tmp = *tr;                                 // plain data: the planner only reads it
+    tmp.sm_count = sm_count;
+    const int pv = fp32 ? 2 : 1;
+    const PersistentPlan pl = plan_persistent(&tmp, n, turns, 2, pv);
+    plan[0] = pl.dynamic; plan[1] = pl.warps_per_smsp; plan[2] = pl.ctas_per_sm; plan[3] = pl.threads;
+    plan[4] = pl.item_turns; plan[5] = pl.flip_on_q ? 1 : 0; plan[6] = (long long)pl.ilp * pv;
+    return LT_OK;
+}
+
+int lt_item_schedule(unsigned int turns, unsigned int item_turns, int taper, unsigned int c,
+                     unsigned int* nchunks, unsigned int* start, unsigned int* len) {
+    if (!nchunks) return LT_E_NULL;
+    if (turns == 0 || item_turns == 0) return LT_E_PARAM;
+    ItemSchedule s;
+    s.init(turns, item_turns, taper);
+    *nchunks = s.nchunks;
+    if (start || len) {
+        if (c >= s.nchunks) return LT_E_PARAM;
+        unsigned int a = 0, b = 0;
+        s.span(c, taper, &a, &b);
+        if (start) *start = a;
+        if (len) *len = b;
+    }
+    return LT_OK;
+}
+
 int lt_probe_fp64(int blocks, int threads, int chains, long long iters, double* rate_host,
                   double* ms_host) {
     if (!rate_host) return LT_E_NULL;

@@ -91,6 +91,10 @@ def _load():
                                   POINTER(c_double)]),
         "lt_probe_pipe": (c_int, [c_int, c_int, c_int, c_int, c_longlong, POINTER(c_double),
                                   POINTER(c_double)]),
+        "lt_plan_fused": (c_int, [vp, sz, ull, c_int, c_int, POINTER(c_longlong)]),
+        "lt_item_schedule": (c_int, [ctypes.c_uint, ctypes.c_uint, c_int, ctypes.c_uint,
+                                     POINTER(ctypes.c_uint), POINTER(ctypes.c_uint),
+                                     POINTER(ctypes.c_uint)]),
         # SURVEY.md sec. 8(f) rows f2-f4
         "lt_track_programme": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp]),
         "lt_track_programme_per_turn": (c_int, [vp, vp, vp, sz, ull, vp, vp, vp, vp, vp]),
@@ -172,6 +176,14 @@ class Tracker:
         v = c_longlong()
         self._check(_lib.lt_get_stat(self._h, stat, byref(v)))
         return v.value
+
+    def plan_fused(self, n: int, turns: int, sm_count: int = 148, fp32: bool = False) -> dict:
+        """Launch shape lt_track_fused would pick (host logic only, no GPU)."""
+        plan = (c_longlong * 7)()
+        self._check(_lib.lt_plan_fused(self._h, n, turns, sm_count, 1 if fp32 else 0, plan))
+        keys = ("dynamic", "warps_per_smsp", "ctas_per_sm", "threads", "item_turns", "flip_on_q",
+                "particles_per_lane")
+        return dict(zip(keys, (int(v) for v in plan)))
 
     # ---- device-pointer calls: z, delta are CUDA tensors (or raw addresses); stream = int
     def track_fused(self, z, delta, n: int, turns: int, stream: int = 0):
@@ -287,6 +299,21 @@ def probe_pipe(kind: int, blocks: int, threads: int, chains: int, iters: int):
     if rc != OK:
         raise LongtrackError(rc)
     return rate.value, mhz.value
+
+
+def item_schedule(turns: int, item_turns: int, taper: bool = True):
+    """[(first turn, length)] of every chunk of a launch (host logic only, no GPU)."""
+    n, a, b = ctypes.c_uint(), ctypes.c_uint(), ctypes.c_uint()
+    rc = _lib.lt_item_schedule(turns, item_turns, 1 if taper else 0, 0, byref(n), None, None)
+    if rc != OK:
+        raise LongtrackError(rc)
+    out = []
+    for c in range(n.value):
+        rc = _lib.lt_item_schedule(turns, item_turns, 1 if taper else 0, c, byref(n), byref(a), byref(b))
+        if rc != OK:
+            raise LongtrackError(rc)
+        out.append((a.value, b.value))
+    return out
 
 
 def strerror(code: int) -> str:

@@ -200,3 +200,56 @@ def test_product_path_never_touches_the_oracle():
             "paper_1610_05801_b200/csrc/, include/longtrack.h", "").replace(
             "from ``paper_1610_05801_b200``", "") or f == "__init__.py"
         assert "longtrack.h\"" not in text and "kernels.cuh" not in text
+
+
+# ---------------------------------------------------------------- host logic: schedule and planner
+@pytest.mark.parametrize("turns,item", [(1, 1), (63, 64), (64, 64), (65, 64), (777, 50), (777, 200), (777, 776),
+                                         (70_000, 2048), (100_000, 2048), (2400, 1024), (2047, 1024), (4096, 1)])
+def test_item_schedule_covers_every_turn_once(lt, turns, item):
+    """The tapered work-item schedule: chunks are contiguous, cover
+    [0, turns) exactly, full items come first, the tail halves down to <= 64 turns, and the
+    plain schedule is ceil(turns / item) equal chunks."""
+    sched = lt.item_schedule(turns, item, taper=True)
+    pos = 0
+    for start, length in sched:
+        assert start == pos and length >= 1
+        pos += length
+    assert pos == turns
+    lens = [l for _, l in sched]
+    nfull = max(turns // item - 1, 0)
+    assert lens[:nfull] == [item] * nfull
+    tail = lens[nfull:]
+    assert all(a >= b for a, b in zip(tail, tail[1:])) or len(tail) <= 1 or tail[-1] <= 64
+    assert tail[-1] <= max(64, 1) or len(tail) == 1
+    assert sum(tail) == turns - nfull * item and sum(tail) < 2 * item + (item if turns < item else 0) + 1
+    plain = lt.item_schedule(turns, item, taper=False)
+    assert len(plain) == -(-turns // item) and sum(l for _, l in plain) == turns
+    assert all(l == item for _, l in plain[:-1])
+
+
+def test_planner_picks_the_measured_launch_shapes(lt):
+    """lt_plan_fused is the host logic behind lt_track_fused (no GPU): at the configs[1] size two
+    particles per lane on 2 warps per sub-partition with every slot busy; at 10^6 particles 4
+    warps; a bunch smaller than one wave gets static slots; options force a shape."""
+    from paper_1610_05801_b200 import workloads as wl
+    tr = lt.Tracker(wl.RING, "leapfrog")
+    p = tr.plan_fused(100_000, 70_000)
+    assert (p["dynamic"], p["particles_per_lane"], p["warps_per_smsp"], p["threads"]) == (1, 2, 2, 256)
+    assert p["item_turns"] == 2048 and p["flip_on_q"] == 0
+    groups, slots = -(-100_000 // 64), 148 * 4 * p["warps_per_smsp"]
+    assert groups > slots                                  # dynamic only when every slot stays busy
+    p = tr.plan_fused(1_000_000, 100_000)
+    assert (p["dynamic"], p["particles_per_lane"], p["warps_per_smsp"]) == (1, 2, 4)
+    p = tr.plan_fused(1_000, 1_000)
+    assert p["dynamic"] == 0 and p["item_turns"] == 0
+    p = tr.plan_fused(1_000_000, 10_000, fp32=True)
+    assert p["particles_per_lane"] in (2, 4)               # packed pairs
+    tr.set_option(lt.OPT_FUSED_ILP, 1)
+    tr.set_option(lt.OPT_WARPS_PER_SMSP, 5)
+    tr.set_option(lt.OPT_FLIP_ON_Q, 1)
+    tr.set_option(lt.OPT_ITEM_TURNS, 300)
+    p = tr.plan_fused(100_000, 70_000)
+    assert (p["particles_per_lane"], p["warps_per_smsp"], p["flip_on_q"], p["item_turns"]) == (1, 5, 1, 300)
+    assert p["threads"] == 640
+    with pytest.raises(lt.LongtrackError):
+        tr.plan_fused(0, 10)
