@@ -420,6 +420,10 @@ def bench_shapes(cx: Ctx) -> dict:
                     cases.append(("ilp%d W%d %s item%d" % (ilp, w, "q" if fq else "f", item),
                                   {lt.OPT_FUSED_MODE: 3, lt.OPT_FUSED_ILP: ilp, lt.OPT_WARPS_PER_SMSP: w,
                                    lt.OPT_FLIP_ON_Q: fq, lt.OPT_ITEM_TURNS: item}))
+            for ilp, w, fq in ((2, 2, 0), (2, 3, 0), (2, 4, 0), (1, 5, 1), (1, 8, 1)):
+                cases.append(("wrap ilp%d W%d %s" % (ilp, w, "q" if fq else "f"),
+                              {lt.OPT_FUSED_MODE: 4, lt.OPT_FUSED_ILP: ilp, lt.OPT_WARPS_PER_SMSP: w,
+                               lt.OPT_FLIP_ON_Q: fq}))
             for w in (4, 8):
                 cases.append(("static ilp2 W%d" % w, {lt.OPT_FUSED_MODE: 2, lt.OPT_FUSED_ILP: 2,
                                                         lt.OPT_WARPS_PER_SMSP: min(w, 4)}))
@@ -433,7 +437,7 @@ def bench_shapes(cx: Ctx) -> dict:
                 for k, v in opts.items():
                     tr.set_option(k, v)
                 sec = cx.timed(lambda: tr.track_fused(z, d, n, turns, cx.sp), 3, flush=False)
-                rows[label] = {"ms": round(1e3 * sec, 3),
+                rows[label] = {"ms": round(1e3 * sec, 3), "mode": tr.get_stat(lt.STAT_LAST_MODE),
                                "frac": round(FP64_INSTR_PER_PT * n * turns / sec / 1e9 / cx.peak_fp64, 4),
                                "block": tr.get_stat(lt.STAT_LAST_BLOCK), "ilp": tr.get_stat(lt.STAT_LAST_ILP),
                                "item": tr.get_stat(lt.STAT_LAST_ITEM_TURNS)}
@@ -703,7 +707,8 @@ def run_cuda(args) -> None:
     fused_launch_s = t_fused / args.steps              # one fused kernel launch per step
     achieved_ginstr = n * turns * FP64_INSTR_PER_PT / fused_launch_s / 1e9
     mode = {1: "fused_kernel (plain)", 2: "fused_persistent_kernel (static slots)",
-            3: "fused_persistent_kernel (dynamic chunk scheduling)"}[tr.get_stat(lt.STAT_LAST_MODE)]
+            3: "fused_persistent_kernel (ticket queue)",
+            4: "fused_persistent_kernel (static wrap-around schedule)"}[tr.get_stat(lt.STAT_LAST_MODE)]
     roofline = {"bound": "alu", "kernel": mode + " <double, leap-frog, single harmonic, merged drifts>",
                 "achieved": achieved_ginstr, "peak": cx.peak_fp64, "unit": "G FP64 instr/s",
                 "frac": achieved_ginstr / cx.peak_fp64,

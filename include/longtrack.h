@@ -143,9 +143,12 @@ enum {
     LT_OPT_PER_TURN_CTAS_PER_SM = 6, /* persistent CTAs per SM of the per-turn kernel      */
     LT_OPT_PER_TURN_REVERSE = 7, /* 1 (default): odd turns walk the arrays backwards so the
                                   tail the previous turn left in L2 is read first          */
-    LT_OPT_FUSED_MODE     = 8, /* 0 (default): planner picks the persistent kernel in static or
-                                  dynamic form; 1: plain one-thread-per-particle kernel
-                                  (LT_OPT_FUSED_ILP / _BLOCK apply); 3: force dynamic        */
+    LT_OPT_FUSED_MODE     = 8, /* 0 (default): planner picks the persistent kernel's schedule;
+                                  1: plain one-thread-per-particle kernel (LT_OPT_FUSED_ILP /
+                                  _BLOCK apply); 2: static slots (group g on slot g mod slots for
+                                  all turns); 3: on-device ticket queue of work items; 4: static
+                                  wrap-around schedule (needs at least as many groups as slots,
+                                  else static slots).  Same bits in every mode.               */
     LT_OPT_ITEM_TURNS     = 9, /* turns per work item of the dynamic persistent kernel
                                   (0 = planner: 128..2048; the last items of a launch are halved
                                   again and again); results do not depend on it                    */
@@ -163,7 +166,7 @@ enum {
     LT_STAT_LAST_BLOCK      = 3,
     LT_STAT_LAST_ILP        = 4, /* particles per lane of the last fused launch             */
     LT_STAT_SM_COUNT        = 5,
-    LT_STAT_LAST_MODE       = 6, /* 1 plain, 2 persistent static, 3 persistent dynamic          */
+    LT_STAT_LAST_MODE       = 6, /* 1 plain, 2 static slots, 3 ticket queue, 4 wrap-around         */
     LT_STAT_LAST_ITEM_TURNS = 7
 };
 

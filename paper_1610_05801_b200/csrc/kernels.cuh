@@ -515,27 +515,16 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
     constexpr unsigned int G = 32u * ILP * L::PV;
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned long long groups = (n + G - 1) / G;
-    ItemSchedule sched;
-    sched.init(turns, item_turns, dynamic);
-    const unsigned int nchunks = sched.nchunks;
-    const unsigned long long total = groups * nchunks;
-    // static mode (few groups): slot s of the grid owns groups s, s + S, ... for all turns;
-    // slots are numbered SM-first so that groups spread evenly over SMs and sub-partitions
     const unsigned long long slots = (unsigned long long)gridDim.x * (blockDim.x >> 5);
-    unsigned long long next = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
-    for (;;) {
-        unsigned long long t = next;
-        if (dynamic) {
-            if (lane == 0) t = atomicAdd(ticket, 1ULL);
-            t = __shfl_sync(0xffffffffu, t, 0);
-        } else {
-            next += slots;
-        }
-        if (t >= total) break;
-        const unsigned int c = (unsigned int)(t / groups);
-        const unsigned long long g = t - (unsigned long long)c * groups;
-        if (c > 0) {
-            while (ld_acquire_u32(done + g) < c) __nanosleep(64);
+    // slots are numbered SM-first so that consecutive slots sit on different SMs
+    const unsigned long long slot = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
+
+    // turns [t_begin, t_begin + nt) of group g: wait until progress word `done[g]` has reached
+    // `need` (0 = nothing to wait for), advance, publish `publish` (0 = nothing follows)
+    auto run_piece = [&](unsigned long long g, unsigned int t_begin, unsigned int nt, unsigned int need,
+                         unsigned int publish) {
+        if (need) {
+            while (ld_acquire_u32(done + g) < need) __nanosleep(64);
         }
         const size_t i0 = (size_t)g * G + lane;
         V x[ILP], dl[ILP];
@@ -548,12 +537,10 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
                 L::set(dl[j], h, (i < n) ? __ldcg(d_arr + i) : T(0));
             }
         }
-        const int first = first_launch && c == 0;
-        const int last = last_launch && c == nchunks - 1;
-        unsigned int t_start, nt;
-        sched.span(c, dynamic, &t_start, &nt);
+        const int first = first_launch && t_begin == 0;
+        const int last = last_launch && t_begin + nt == turns;
         advance<V, INTEG, HARM, SPLIT, ILP, FQ, PROG>(
-            x, dl, nt, first, last, P, PROG ? prog + t_start : nullptr,
+            x, dl, nt, first, last, P, PROG ? prog + t_begin : nullptr,
             PROG ? reinterpret_cast<double2*>(residency_cap) + (threadIdx.x & ~31u) : nullptr);
 #pragma unroll
         for (int j = 0; j < ILP; ++j) {
@@ -563,11 +550,58 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
                 if (i < n) { __stcg(z_arr + i, L::get(x[j], h)); __stcg(d_arr + i, L::get(dl[j], h)); }
             }
         }
-        if (nchunks > 1) {
+        if (publish) {
             __threadfence();
             __syncwarp();
-            if (lane == 0) st_release_u32(done + g, c + 1);
+            if (lane == 0) st_release_u32(done + g, publish);
         }
+    };
+
+    if (dynamic == 2) {
+        // WRAP-AROUND schedule (McNaughton's rule for preemptive scheduling on identical machines):
+        // the work of the launch is the line x in [0, groups * turns), group-major; slot s owns
+        // [s X / S, (s+1) X / S) and walks it from the top down, piece by piece.  Its first piece
+        // is the EARLY part of a group (turns 0 .. t), its last piece the LATE part of another
+        // (turns t' .. end) whose early part was the first piece of slot s - 1: with groups >=
+        // slots a group is cut at most once, the late part starts groups/slots - 1 group-runs
+        // after the early one ended, and every slot finishes at the same moment -- no ticket, no
+        // tail, two or three item switches per warp instead of dozens.  All FP64 timing is
+        // data-independent and every sub-partition holds the same number of warps, which is
+        // what makes a static preemptive schedule exact here.
+        const unsigned __int128 X = (unsigned __int128)groups * turns;
+        const unsigned long long x_lo = (unsigned long long)(X * slot / slots);
+        unsigned long long x = (unsigned long long)(X * (slot + 1) / slots);
+        while (x > x_lo) {
+            const unsigned long long g = (x - 1) / turns;
+            const unsigned long long gx = g * (unsigned long long)turns;
+            const unsigned int t_end = (unsigned int)(x - gx);
+            const unsigned int t_begin = x_lo > gx ? (unsigned int)(x_lo - gx) : 0u;
+            run_piece(g, t_begin, t_end - t_begin, t_begin ? 1u : 0u, t_end < turns ? 1u : 0u);
+            x = gx + t_begin;
+        }
+        return;
+    }
+
+    ItemSchedule sched;
+    sched.init(turns, item_turns, dynamic);
+    const unsigned int nchunks = sched.nchunks;
+    const unsigned long long total = groups * nchunks;
+    // static mode (few groups): slot s of the grid owns groups s, s + S, ... for all turns
+    unsigned long long next = slot;
+    for (;;) {
+        unsigned long long t = next;
+        if (dynamic) {
+            if (lane == 0) t = atomicAdd(ticket, 1ULL);
+            t = __shfl_sync(0xffffffffu, t, 0);
+        } else {
+            next += slots;
+        }
+        if (t >= total) break;
+        const unsigned int c = (unsigned int)(t / groups);
+        const unsigned long long g = t - (unsigned long long)c * groups;
+        unsigned int t_start, nt;
+        sched.span(c, dynamic, &t_start, &nt);
+        run_piece(g, t_start, nt, c, nchunks > 1 ? c + 1 : 0u);
     }
 }
 

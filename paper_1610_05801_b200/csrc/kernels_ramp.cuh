@@ -233,13 +233,59 @@ ramp_persistent_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, s
     constexpr unsigned int G = 32u * ILP;
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned long long groups = (n + G - 1) / G;
+    const unsigned long long slots = (unsigned long long)gridDim.x * (blockDim.x >> 5);
+    const unsigned long long slot = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
+    double2* stage = reinterpret_cast<double2*>(ramp_smem) + 192u * (threadIdx.x >> 5);
+
+    // sub-steps [s_begin, s_begin + ns) of group g (see run_piece in kernels.cuh)
+    auto run_piece = [&](unsigned long long g, unsigned int s_begin, unsigned int ns, unsigned int need,
+                         unsigned int publish) {
+        if (need) {
+            while (ld_acquire_u32(done + g) < need) __nanosleep(64);
+        }
+        const size_t i0 = (size_t)g * G + lane;
+        double x[ILP], dl[ILP];
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            const size_t i = i0 + 32u * j;
+            x[j] = (i < n) ? __ldcg(z_arr + i) : 0.0;
+            dl[j] = (i < n) ? __ldcg(d_arr + i) : 0.0;
+        }
+        const int first = first_launch && s_begin == 0;
+        const int last = last_launch && s_begin + ns == nsteps;
+        ramp_advance<HARM, SPLIT, ILP>(x, dl, ns, first, last, P, table + 3 * (size_t)s_begin, stage);
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            const size_t i = i0 + 32u * j;
+            if (i < n) { __stcg(z_arr + i, x[j]); __stcg(d_arr + i, dl[j]); }
+        }
+        if (publish) {
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) st_release_u32(done + g, publish);
+        }
+    };
+
+    if (dynamic == 2) {                       // wrap-around schedule, see fused_persistent_kernel
+        const unsigned __int128 X = (unsigned __int128)groups * nsteps;
+        const unsigned long long x_lo = (unsigned long long)(X * slot / slots);
+        unsigned long long x = (unsigned long long)(X * (slot + 1) / slots);
+        while (x > x_lo) {
+            const unsigned long long g = (x - 1) / nsteps;
+            const unsigned long long gx = g * (unsigned long long)nsteps;
+            const unsigned int s_end = (unsigned int)(x - gx);
+            const unsigned int s_begin = x_lo > gx ? (unsigned int)(x_lo - gx) : 0u;
+            run_piece(g, s_begin, s_end - s_begin, s_begin ? 1u : 0u, s_end < nsteps ? 1u : 0u);
+            x = gx + s_begin;
+        }
+        return;
+    }
+
     ItemSchedule sched;
     sched.init(nsteps, item_steps, dynamic);
     const unsigned int nchunks = sched.nchunks;
     const unsigned long long total = groups * nchunks;
-    const unsigned long long slots = (unsigned long long)gridDim.x * (blockDim.x >> 5);
-    unsigned long long next = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
-    double2* stage = reinterpret_cast<double2*>(ramp_smem) + 192u * (threadIdx.x >> 5);
+    unsigned long long next = slot;
     for (;;) {
         unsigned long long t = next;
         if (dynamic) {
@@ -251,32 +297,9 @@ ramp_persistent_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, s
         if (t >= total) break;
         const unsigned int c = (unsigned int)(t / groups);
         const unsigned long long g = t - (unsigned long long)c * groups;
-        if (c > 0) {
-            while (ld_acquire_u32(done + g) < c) __nanosleep(64);
-        }
-        const size_t i0 = (size_t)g * G + lane;
-        double x[ILP], dl[ILP];
-#pragma unroll
-        for (int j = 0; j < ILP; ++j) {
-            const size_t i = i0 + 32u * j;
-            x[j] = (i < n) ? __ldcg(z_arr + i) : 0.0;
-            dl[j] = (i < n) ? __ldcg(d_arr + i) : 0.0;
-        }
-        const int first = first_launch && c == 0;
-        const int last = last_launch && c == nchunks - 1;
         unsigned int s_start, ns;
         sched.span(c, dynamic, &s_start, &ns);
-        ramp_advance<HARM, SPLIT, ILP>(x, dl, ns, first, last, P, table + 3 * (size_t)s_start, stage);
-#pragma unroll
-        for (int j = 0; j < ILP; ++j) {
-            const size_t i = i0 + 32u * j;
-            if (i < n) { __stcg(z_arr + i, x[j]); __stcg(d_arr + i, dl[j]); }
-        }
-        if (nchunks > 1) {
-            __threadfence();
-            __syncwarp();
-            if (lane == 0) st_release_u32(done + g, c + 1);
-        }
+        run_piece(g, s_start, ns, c, nchunks > 1 ? c + 1 : 0u);
     }
 }
 

@@ -242,11 +242,20 @@ PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long lon
             const unsigned long long slots = (unsigned long long)sms * 4 * w;
             for (int fq = 0; fq < 2; ++fq) {
                 if (tr->flip_on_q >= 0 && fq != tr->flip_on_q) continue;
-                for (int dyn = 0; dyn < 2; ++dyn) {
+                for (int dyn = 0; dyn < 3; ++dyn) {          // 0 static, 1 ticket queue, 2 wrap-around
                     double score;
-                    if (dyn) {                               // every slot busy until the tail
+                    // measured (profiles/r2_fused_shapes.md): with 2 warps per sub-partition the ticket
+                    // queue costs 1.5 % (an item switch halves the sub-partition's rate, dozens of
+                    // switches per warp, tapered tail) and the wrap-around schedule nothing; from 3
+                    // warps on the queue's switches hide behind the other warps and its dynamic
+                    // balancing is worth 0.3 % over the static schedule
+                    if (dyn == 2) {                          // static pre-emptive schedule: no queue, no tail
+                        if (groups < slots) continue;
+                        score = (w <= 2 ? 1.0 : 0.994) * loop_rate(ilp, w, fq);
+                    } else if (dyn == 1) {                   // ticket queue: every slot busy until the tail
                         if (groups <= slots && tr->fused_mode != 3) continue;
-                        score = loop_rate(ilp, w, fq);
+                        score = (w <= 2 ? 0.985 : 0.997) * loop_rate(ilp, w, fq);
+                        if (groups < slots) score *= (double)groups / (double)slots;   // forced: idle warps
                     } else if (groups <= slots) {            // one wave: busiest sub-partition rules
                         const double per_smsp = std::ceil(avg);
                         if (tr->warps_per_smsp == 0 && (double)w != std::min(per_smsp, ilp == 2 ? 4.0 : 16.0)) continue;
@@ -255,8 +264,9 @@ PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long lon
                         const double rounds = std::ceil((double)groups / (double)slots);
                         score = loop_rate(ilp, w, fq) * avg / (rounds * w);
                     }
-                    if (tr->fused_mode == 3 && !dyn) continue;
-                    if (tr->fused_mode == 2 && dyn) continue;
+                    if (tr->fused_mode == 4 && dyn != 2) continue;
+                    if (tr->fused_mode == 3 && dyn != 1) continue;
+                    if (tr->fused_mode == 2 && dyn != 0) continue;
                     if (score > best_score) {
                         best_score = score;
                         best.dynamic = dyn;
@@ -270,7 +280,12 @@ PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long lon
             }
         }
     }
-    if (best.dynamic) {
+    if (best_score < 0.0) {                                  // forced wrap-around with fewer groups than slots
+        lt_tracker relaxed = *tr;
+        relaxed.fused_mode = 2;
+        return plan_persistent(&relaxed, n, turns, max_ilp, pv);
+    }
+    if (best.dynamic == 1) {
         // an item switch costs a warp about 3 us (ticket, progress word, state load; store, fence,
         // release), during which its sub-partition runs at half rate when it holds two warps: long
         // items (2048 turns = 120 us) amortise that, and the tapered tail of the schedule
@@ -363,8 +378,8 @@ int track_fused_persistent(lt_tracker* tr, T* z, T* d, size_t n, unsigned long l
     while (done < turns) {
         unsigned long long chunk = std::min<unsigned long long>(turns - done, (unsigned long long)tr->chunk_turns);
         const int first = done == 0, last = done + chunk == turns;
-        const unsigned int item = pl.dynamic ? std::min<unsigned int>(pl.item_turns, (unsigned int)chunk) : (unsigned int)chunk;
-        if (pl.dynamic) {
+        const unsigned int item = pl.dynamic == 1 ? std::min<unsigned int>(pl.item_turns, (unsigned int)chunk) : (unsigned int)chunk;
+        if (pl.dynamic) {                                    // ticket + progress words of this launch
             LT_CUDA(tr, cudaMemsetAsync(tr->sched, 0, 8 + 4 * ((n + 31) / 32), st));
         }
         cudaError_t e;
@@ -385,8 +400,8 @@ int track_fused_persistent(lt_tracker* tr, T* z, T* d, size_t n, unsigned long l
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
     tr->last_ilp = pl.ilp * kPV;
-    tr->last_mode = pl.dynamic ? 3 : 2;
-    tr->last_item_turns = pl.dynamic ? pl.item_turns : 0;
+    tr->last_mode = pl.dynamic == 2 ? 4 : (pl.dynamic ? 3 : 2);
+    tr->last_item_turns = pl.dynamic == 1 ? pl.item_turns : 0;
     return LT_OK;
 }
 
@@ -708,7 +723,7 @@ int lt_set_option(lt_tracker* tr, int option, long long value) {
             tr->per_turn_ctas_per_sm = value; return LT_OK;
         case LT_OPT_PER_TURN_REVERSE: tr->per_turn_reverse = value != 0; return LT_OK;
         case LT_OPT_FUSED_MODE:
-            if (value < 0 || value > 3) return LT_E_PARAM;
+            if (value < 0 || value > 4) return LT_E_PARAM;
             tr->fused_mode = value; return LT_OK;
         case LT_OPT_ITEM_TURNS:
             if (value < 0 || value > (1LL << 31) - 1) return LT_E_PARAM;

@@ -95,8 +95,8 @@ int track_programme_fused(lt_tracker* tr, double* z, double* d, size_t n, unsign
     while (done < turns) {
         const unsigned long long chunk = std::min<unsigned long long>(turns - done, chunk_max);
         const int first = done == 0, last = done + chunk == turns;
-        const unsigned int item = pl.dynamic ? std::min<unsigned int>(pl.item_turns, (unsigned int)chunk)
-                                             : (unsigned int)chunk;
+        const unsigned int item = pl.dynamic == 1 ? std::min<unsigned int>(pl.item_turns, (unsigned int)chunk)
+                                                  : (unsigned int)chunk;
         // the table of the previous chunk is free again: its kernel precedes this one on the stream
         programme_pack_kernel<<<(unsigned)((chunk + 255) / 256), 256, 0, st>>>(
             volt, phase, done, (unsigned int)chunk, turns, kInvPi, split ? 0 : 1, tr->prog_table);
@@ -120,8 +120,8 @@ int track_programme_fused(lt_tracker* tr, double* z, double* d, size_t n, unsign
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
     tr->last_ilp = pl.ilp;
-    tr->last_mode = pl.dynamic ? 3 : 2;
-    tr->last_item_turns = pl.dynamic ? pl.item_turns : 0;
+    tr->last_mode = pl.dynamic == 2 ? 4 : (pl.dynamic ? 3 : 2);
+    tr->last_item_turns = pl.dynamic == 1 ? pl.item_turns : 0;
     return LT_OK;
 }
 
@@ -325,8 +325,9 @@ TransPlan plan_transverse(const lt_tracker* tr, size_t n, unsigned long long tur
     tp.ilp = ilp;
     const unsigned long long groups = (n + 32 * ilp - 1) / (32 * ilp);
     PersistentPlan pl = {0, 4, 1, 512, 0, true, 1};
-    pl.dynamic = (groups > slots || tr->fused_mode == 3) && tr->fused_mode != 2;
-    if (pl.dynamic) {
+    // more groups than slots: the wrap-around static schedule (or the ticket queue if forced)
+    pl.dynamic = tr->fused_mode == 2 ? 0 : (tr->fused_mode == 3 ? 1 : (groups >= slots ? 2 : 0));
+    if (pl.dynamic == 1) {
         unsigned long long it = tr->item_turns > 0
                                     ? (unsigned long long)tr->item_turns
                                     : std::min<unsigned long long>(2048, std::max<unsigned long long>(128, turns / 8));
@@ -416,7 +417,7 @@ int track_transverse_fused(lt_tracker* tr, double* x, double* xp, double* y, dou
     while (done < turns) {
         const unsigned long long chunk = std::min<unsigned long long>(turns - done, (unsigned long long)tr->chunk_turns);
         const int first = done == 0, last = done + chunk == turns;
-        const unsigned int item = pl.dynamic ? std::min<unsigned int>(pl.item_turns, (unsigned int)chunk) : (unsigned int)chunk;
+        const unsigned int item = pl.dynamic == 1 ? std::min<unsigned int>(pl.item_turns, (unsigned int)chunk) : (unsigned int)chunk;
         if (pl.dynamic) LT_CUDA(tr, cudaMemsetAsync(tr->sched, 0, 8 + 4 * ((n + 31) / 32), st));
         cudaError_t e = longi ? launch_transverse<true>(x, xp, y, yp, z, d, n, (unsigned)chunk, item, first, last, tp, tr, st)
                               : launch_transverse<false>(x, xp, y, yp, z, d, n, (unsigned)chunk, item, first, last, tp, tr, st);
@@ -431,8 +432,8 @@ int track_transverse_fused(lt_tracker* tr, double* x, double* xp, double* y, dou
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
     tr->last_ilp = tp.ilp;
-    tr->last_mode = pl.dynamic ? 3 : 2;
-    tr->last_item_turns = pl.dynamic ? pl.item_turns : 0;
+    tr->last_mode = pl.dynamic == 2 ? 4 : (pl.dynamic ? 3 : 2);
+    tr->last_item_turns = pl.dynamic == 1 ? pl.item_turns : 0;
     return LT_OK;
 }
 

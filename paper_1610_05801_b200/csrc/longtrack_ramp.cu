@@ -157,7 +157,7 @@ int lt_track_ramp(lt_tracker* tr, double* z, double* d, size_t n, unsigned long 
         const unsigned long long chunk = std::min<unsigned long long>(turns - done, chunk_max);
         const int first = done == 0, last = done + chunk == turns;
         const unsigned int item_turns =
-            pl.dynamic ? std::min<unsigned int>(pl.item_turns, (unsigned int)chunk) : (unsigned int)chunk;
+            pl.dynamic == 1 ? std::min<unsigned int>(pl.item_turns, (unsigned int)chunk) : (unsigned int)chunk;
         // the table of the previous chunk is free again: its kernel precedes this one on the stream
         ramp_pack_kernel<<<(unsigned)((chunk + 255) / 256), 256, 0, st>>>(
             p0c, volt, phase, done, (unsigned int)chunk, turns, tr->p.integrator, split ? 0 : 1, R,
@@ -179,8 +179,8 @@ int lt_track_ramp(lt_tracker* tr, double* z, double* d, size_t n, unsigned long 
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
     tr->last_ilp = pl.ilp;
-    tr->last_mode = pl.dynamic ? 3 : 2;
-    tr->last_item_turns = pl.dynamic ? pl.item_turns : 0;
+    tr->last_mode = pl.dynamic == 2 ? 4 : (pl.dynamic ? 3 : 2);
+    tr->last_item_turns = pl.dynamic == 1 ? pl.item_turns : 0;
     return LT_OK;
 }
 

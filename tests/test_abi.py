@@ -88,7 +88,7 @@ def test_options_and_stats(lt):
     tr.set_option(lt.OPT_CHUNK_TURNS, 1000)
     assert tr.get_option(lt.OPT_CHUNK_TURNS) == 1000
     for opt, bad in ((lt.OPT_CHUNK_TURNS, 0), (lt.OPT_FUSED_ILP, 3), (lt.OPT_FUSED_BLOCK, 100),
-                     (lt.OPT_PER_TURN_CTAS_PER_SM, 0), (lt.OPT_FUSED_MODE, 4),
+                     (lt.OPT_PER_TURN_CTAS_PER_SM, 0), (lt.OPT_FUSED_MODE, 5),
                      (lt.OPT_WARPS_PER_SMSP, 9), (lt.OPT_FLIP_ON_Q, 2), (99, 1)):
         with pytest.raises(lt.LongtrackError) as e:
             tr.set_option(opt, bad)
@@ -233,13 +233,19 @@ def test_planner_picks_the_measured_launch_shapes(lt):
     warps; a bunch smaller than one wave gets static slots; options force a shape."""
     from paper_1610_05801_b200 import workloads as wl
     tr = lt.Tracker(wl.RING, "leapfrog")
-    p = tr.plan_fused(100_000, 70_000)
-    assert (p["dynamic"], p["particles_per_lane"], p["warps_per_smsp"], p["threads"]) == (1, 2, 2, 256)
-    assert p["item_turns"] == 2048 and p["flip_on_q"] == 0
+    p = tr.plan_fused(100_000, 70_000)                     # 2 = static wrap-around schedule
+    assert (p["dynamic"], p["particles_per_lane"], p["warps_per_smsp"], p["threads"]) == (2, 2, 2, 256)
+    assert p["item_turns"] == 0 and p["flip_on_q"] == 0
     groups, slots = -(-100_000 // 64), 148 * 4 * p["warps_per_smsp"]
-    assert groups > slots                                  # dynamic only when every slot stays busy
-    p = tr.plan_fused(1_000_000, 100_000)
-    assert (p["dynamic"], p["particles_per_lane"], p["warps_per_smsp"]) == (1, 2, 4)
+    assert groups >= slots                                 # only when every slot stays busy
+    p = tr.plan_fused(1_000_000, 100_000)                  # many groups per slot: the ticket queue
+    assert (p["dynamic"], p["particles_per_lane"], p["warps_per_smsp"], p["item_turns"]) == (1, 2, 4, 2048)
+    tr.set_option(lt.OPT_FUSED_MODE, lt.FUSED_PERSISTENT_DYNAMIC)
+    p = tr.plan_fused(100_000, 70_000)                     # the ticket queue when forced
+    assert (p["dynamic"], p["particles_per_lane"], p["warps_per_smsp"], p["item_turns"]) == (1, 2, 2, 2048)
+    tr.set_option(lt.OPT_FUSED_MODE, lt.FUSED_PERSISTENT_WRAP)
+    assert tr.plan_fused(1_000, 1_000)["dynamic"] == 0     # fewer groups than slots: static slots
+    tr.set_option(lt.OPT_FUSED_MODE, lt.FUSED_AUTO)
     p = tr.plan_fused(1_000, 1_000)
     assert p["dynamic"] == 0 and p["item_turns"] == 0
     p = tr.plan_fused(1_000_000, 10_000, fp32=True)
@@ -248,6 +254,7 @@ def test_planner_picks_the_measured_launch_shapes(lt):
     tr.set_option(lt.OPT_WARPS_PER_SMSP, 5)
     tr.set_option(lt.OPT_FLIP_ON_Q, 1)
     tr.set_option(lt.OPT_ITEM_TURNS, 300)
+    tr.set_option(lt.OPT_FUSED_MODE, lt.FUSED_PERSISTENT_DYNAMIC)
     p = tr.plan_fused(100_000, 70_000)
     assert (p["particles_per_lane"], p["warps_per_smsp"], p["flip_on_q"], p["item_turns"]) == (1, 5, 1, 300)
     assert p["threads"] == 640

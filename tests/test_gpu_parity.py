@@ -111,6 +111,16 @@ def test_dynamic_scheduling_is_bit_identical_to_the_plain_kernel(integrator, rat
                 tr.set_option(lt.OPT_ITEM_TURNS, item)
                 out = gpu_track(tr, z0, d0, 777)
                 assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1]), (split, ilp, item)
+        tr.set_option(lt.OPT_FUSED_MODE, lt.FUSED_PERSISTENT_WRAP)     # static wrap-around schedule
+        for ilp, w in ((1, 1), (1, 5), (2, 1), (2, 3), (0, 0)):        # 150 001 particles: groups > slots
+            tr.set_option(lt.OPT_FUSED_ILP, ilp)
+            tr.set_option(lt.OPT_WARPS_PER_SMSP, w)
+            out = gpu_track(tr, z0, d0, 777)
+            assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1]), (split, "wrap", ilp, w)
+            assert tr.get_stat(lt.STAT_LAST_MODE) == lt.FUSED_PERSISTENT_WRAP
+        tr.set_option(lt.OPT_WARPS_PER_SMSP, 0)
+        tr.set_option(lt.OPT_FUSED_ILP, 0)
+        tr.set_option(lt.OPT_FUSED_MODE, lt.FUSED_PERSISTENT_DYNAMIC)
         tr.set_option(lt.OPT_CHUNK_TURNS, 300)          # several launches, each with its own items
         out = gpu_track(tr, z0, d0, 777)
         assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1])
@@ -152,14 +162,20 @@ def test_ragged_sizes_all_layouts(n):
                                   (lt.FUSED_PERSISTENT_DYNAMIC, 5 if ilp == 1 else 3, 7, 0),
                                   (lt.FUSED_PERSISTENT_DYNAMIC, 8 if ilp == 1 else 4, 33, 1),
                                   (lt.FUSED_PERSISTENT_DYNAMIC, 2, 1, 1),
-                                  (lt.FUSED_PERSISTENT_DYNAMIC, 12 if ilp == 1 else 1, 100, 0)):
+                                  (lt.FUSED_PERSISTENT_DYNAMIC, 12 if ilp == 1 else 1, 100, 0),
+                                  (lt.FUSED_PERSISTENT_WRAP, 1, 0, 0), (lt.FUSED_PERSISTENT_WRAP, 2, 0, 1),
+                                  (lt.FUSED_PERSISTENT_WRAP, 0, 0, -1)):
             tr.set_option(lt.OPT_FUSED_MODE, mode)
             tr.set_option(lt.OPT_WARPS_PER_SMSP, w)
             tr.set_option(lt.OPT_ITEM_TURNS, item)
             tr.set_option(lt.OPT_FLIP_ON_Q, fq)
             zg, dg = gpu_track(tr, z0, d0, 100)
             assert np.array_equal(zg, zr) and np.array_equal(dg, dr), (ilp, mode, w, item, fq)
-            assert tr.get_stat(lt.STAT_LAST_MODE) == mode and tr.get_stat(lt.STAT_LAST_ILP) == ilp
+            groups_lt_slots = -(-n // (32 * ilp)) < 148 * 4 * max(w, 1)     # wrap needs groups >= slots
+            want = lt.FUSED_PERSISTENT_STATIC if (mode == lt.FUSED_PERSISTENT_WRAP and groups_lt_slots and w) else mode
+            if not (mode == lt.FUSED_PERSISTENT_WRAP and w == 0):
+                assert tr.get_stat(lt.STAT_LAST_MODE) == want, (ilp, mode, w)
+            assert tr.get_stat(lt.STAT_LAST_ILP) == ilp
     zg, dg, mg = gpu_track(tr, z0, d0, 100, "per_turn", want_moments=True)
     assert_particle_gate(p, z0, d0, zg, dg, zo, do, sd, gate=1e-10)
     mo = oracle.moments_of(p, zo, do)

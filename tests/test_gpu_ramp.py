@@ -140,7 +140,8 @@ def test_ramp_every_launch_shape_returns_the_same_bits(integrator):
         for mode, ilp, w, item in ((lt.FUSED_PERSISTENT_DYNAMIC, 1, 14, 40), (lt.FUSED_PERSISTENT_DYNAMIC, 1, 16, 0),
                                    (lt.FUSED_PERSISTENT_STATIC, 1, 16, 0), (lt.FUSED_PERSISTENT_DYNAMIC, 1, 8, 100),
                                    (lt.FUSED_PERSISTENT_DYNAMIC, 2, 1, 64), (lt.FUSED_PERSISTENT_DYNAMIC, 2, 4, 0),
-                                   (lt.FUSED_PERSISTENT_STATIC, 2, 3, 0), (lt.FUSED_PERSISTENT_DYNAMIC, 1, 3, 7)):
+                                   (lt.FUSED_PERSISTENT_STATIC, 2, 3, 0), (lt.FUSED_PERSISTENT_DYNAMIC, 1, 3, 7),
+                                   (lt.FUSED_PERSISTENT_WRAP, 1, 2, 0), (lt.FUSED_PERSISTENT_WRAP, 2, 1, 0)):
             tr.set_option(lt.OPT_FUSED_MODE, mode)
             tr.set_option(lt.OPT_FUSED_ILP, ilp)
             tr.set_option(lt.OPT_WARPS_PER_SMSP, w)
