@@ -369,18 +369,31 @@ transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp
     constexpr unsigned int G = 32u * ILP;
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned long long groups = (n + G - 1) / G;
+    ItemSchedule sched;
+    sched.init(turns, item_turns, dynamic);
+    const unsigned int nchunks = sched.nchunks;
+    const unsigned long long total = groups * nchunks;
     const unsigned long long slots = (unsigned long long)gridDim.x * (blockDim.x >> 5);
-    const unsigned long long slot = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
-
-    // turns [t_begin, t_begin + nt) of group g (see run_piece in kernels.cuh)
-    auto run_piece = [&](unsigned long long g, unsigned int t_begin, unsigned int nt, unsigned int need,
-                         unsigned int publish) {
-        if (need) {
-            while (ld_acquire_u32(done + g) < need) __nanosleep(64);
+    unsigned long long next = (unsigned long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x;
+    for (;;) {
+        unsigned long long t = next;
+        if (dynamic) {
+            if (lane == 0) t = atomicAdd(ticket, 1ULL);
+            t = __shfl_sync(0xffffffffu, t, 0);
+        } else {
+            next += slots;
+        }
+        if (t >= total) break;
+        const unsigned int c = (unsigned int)(t / groups);
+        const unsigned long long g = t - (unsigned long long)c * groups;
+        if (c > 0) {
+            while (ld_acquire_u32(done + g) < c) __nanosleep(64);
         }
         const size_t i0 = (size_t)g * G + lane;
-        const int first = first_launch && t_begin == 0;
-        const int last = last_launch && t_begin + nt == turns;
+        const int first = first_launch && c == 0;
+        const int last = last_launch && c == nchunks - 1;
+        unsigned int t_start, nt;
+        sched.span(c, dynamic, &t_start, &nt);
         double u[ILP][4], v[ILP], dl[ILP];
 #pragma unroll
         for (int j = 0; j < ILP; ++j) {
@@ -420,47 +433,11 @@ transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp
                 if (LONGI) { __stcg(z_arr + i, v[j]); __stcg(d_arr + i, dl[j]); }
             }
         }
-        if (publish) {
+        if (nchunks > 1) {
             __threadfence();
             __syncwarp();
-            if (lane == 0) st_release_u32(done + g, publish);
+            if (lane == 0) st_release_u32(done + g, c + 1);
         }
-    };
-
-    if (dynamic == 2) {                       // wrap-around schedule, see fused_persistent_kernel
-        const unsigned __int128 X = (unsigned __int128)groups * turns;
-        const unsigned long long x_lo = (unsigned long long)(X * slot / slots);
-        unsigned long long x = (unsigned long long)(X * (slot + 1) / slots);
-        while (x > x_lo) {
-            const unsigned long long g = (x - 1) / turns;
-            const unsigned long long gx = g * (unsigned long long)turns;
-            const unsigned int t_end = (unsigned int)(x - gx);
-            const unsigned int t_begin = x_lo > gx ? (unsigned int)(x_lo - gx) : 0u;
-            run_piece(g, t_begin, t_end - t_begin, t_begin ? 1u : 0u, t_end < turns ? 1u : 0u);
-            x = gx + t_begin;
-        }
-        return;
-    }
-
-    ItemSchedule sched;
-    sched.init(turns, item_turns, dynamic);
-    const unsigned int nchunks = sched.nchunks;
-    const unsigned long long total = groups * nchunks;
-    unsigned long long next = slot;
-    for (;;) {
-        unsigned long long t = next;
-        if (dynamic) {
-            if (lane == 0) t = atomicAdd(ticket, 1ULL);
-            t = __shfl_sync(0xffffffffu, t, 0);
-        } else {
-            next += slots;
-        }
-        if (t >= total) break;
-        const unsigned int c = (unsigned int)(t / groups);
-        const unsigned long long g = t - (unsigned long long)c * groups;
-        unsigned int t_start, nt;
-        sched.span(c, dynamic, &t_start, &nt);
-        run_piece(g, t_start, nt, c, nchunks > 1 ? c + 1 : 0u);
     }
 }
 

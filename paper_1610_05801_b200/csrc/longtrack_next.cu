@@ -320,16 +320,22 @@ TransPlan plan_transverse(const lt_tracker* tr, size_t n, unsigned long long tur
     else ilp = 1;
     if (ilp == 1) {
         tp.pl = plan_persistent(tr, n, turns);
+        if (tp.pl.dynamic == 2) {                            // this kernel has no wrap-around schedule
+            tp.pl.dynamic = 1;
+            const unsigned long long it = tr->item_turns > 0
+                                              ? (unsigned long long)tr->item_turns
+                                              : std::min<unsigned long long>(2048, std::max<unsigned long long>(128, turns / 8));
+            tp.pl.item_turns = (unsigned int)std::min<unsigned long long>(it, turns);
+        }
         return tp;
     }
     tp.ilp = ilp;
     const unsigned long long groups = (n + 32 * ilp - 1) / (32 * ilp);
     PersistentPlan pl = {0, 4, 1, 512, 0, true, 1};
-    // more groups than slots: the ticket queue (4 warps per sub-partition hide its item switches;
-    // the wrap-around static schedule measured 1.2 points lower here), wrap-around only if forced
-    pl.dynamic = tr->fused_mode == 2 ? 0
-               : (tr->fused_mode == 4 && groups >= slots) ? 2
-               : (groups > slots || tr->fused_mode == 3) ? 1 : 0;
+    // more groups than slots: the ticket queue (4 warps per sub-partition hide its item switches; the
+    // wrap-around static schedule measured 1.2 points lower and its code cost the kernel a register
+    // spill, so this kernel does not carry it: LT_OPT_FUSED_MODE = 4 means the queue here)
+    pl.dynamic = tr->fused_mode == 2 ? 0 : ((groups > slots || tr->fused_mode >= 3) ? 1 : 0);
     if (pl.dynamic == 1) {
         unsigned long long it = tr->item_turns > 0
                                     ? (unsigned long long)tr->item_turns
