@@ -809,9 +809,13 @@ def main():
     if args.impl == "reference":
         run_reference(args)                              # builds and maps oracle/ only
         return
-    import __graft_entry__ as entry
     if int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        import __graft_entry__ as entry
         entry.build()
+    else:                                               # torchrun: local rank 0 builds, the others wait
+        from paper_1610_05801_b200 import build as lt_build
+        lt_build.wait_until_built()
+        time.sleep(1.0)                                 # let the linker finish writing
     run_cuda(args)
 
 

@@ -45,5 +45,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def wait_until_built(timeout_s: float = 900.0) -> str:
+    """For the ranks of a torchrun launch that do NOT build: block until rank 0's build is there."""
+    import time
+    t0 = time.time()
+    newest = max(os.path.getmtime(p) for p in DEPS)
+    while not (os.path.exists(LIB) and os.path.getmtime(LIB) >= newest):
+        if time.time() - t0 > timeout_s:
+            raise RuntimeError("liblongtrack.so was not built within %.0f s" % timeout_s)
+        time.sleep(0.5)
+    return LIB
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

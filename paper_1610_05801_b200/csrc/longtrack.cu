@@ -251,6 +251,7 @@ PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long lon
                     // balancing is worth 0.3 % over the static schedule
                     if (dyn == 2) {                          // static pre-emptive schedule: no queue, no tail
                         if (groups < slots) continue;
+                        if (groups > (1ULL << 31)) continue;   // groups x turns must stay below 2^63
                         score = (w <= 2 ? 1.0 : 0.994) * loop_rate(ilp, w, fq);
                     } else if (dyn == 1) {                   // ticket queue: every slot busy until the tail
                         if (groups <= slots && tr->fused_mode != 3) continue;
