@@ -110,6 +110,37 @@ def test_programme_split_drift_fused_equals_per_turn_bits_and_chunking_is_invisi
     assert np.array_equal(zs, zt) and np.array_equal(ds, dt)
 
 
+@pytest.mark.parametrize("integrator,ratio2", [("leapfrog", 0.0), ("ruth4", 0.5)])
+def test_programme_every_schedule_and_lane_count_returns_the_same_bits(integrator, ratio2):
+    """Static slots, ticket queue (tapered items) and the wrap-around schedule, one and two
+    particles per lane, at a size with more groups than warp slots (80 003 particles): the fused
+    RF-programme kernel returns the bits of the planner's launch, merged and split drifts, also
+    when the call is cut into several launches."""
+    tr, p = both(integrator, ratio2)
+    z0, d0 = wl.gaussian_bunch(80_003, 0.23, 25, ratio2=ratio2)
+    a, psi = strong_programme(211)
+    zo, do = oracle.track_programme(p, z0, d0, a, psi)
+    for split in (0, 1):
+        tr.set_option(lt.OPT_SPLIT_DRIFTS, split)
+        for opt in (lt.OPT_FUSED_MODE, lt.OPT_FUSED_ILP, lt.OPT_WARPS_PER_SMSP, lt.OPT_ITEM_TURNS):
+            tr.set_option(opt, 0)
+        tr.set_option(lt.OPT_CHUNK_TURNS, 1 << 22)
+        ref = gpu_programme(tr, z0, d0, a, psi, "fused")
+        assert np.abs(ref[0] - zo).max() / oracle.derive(p)["z_max"] <= 1e-10
+        for mode, ilp, w, item, chunk in ((lt.FUSED_PERSISTENT_WRAP, 2, 2, 0, 1 << 22), (lt.FUSED_PERSISTENT_WRAP, 1, 3, 0, 1 << 22),
+                                          (lt.FUSED_PERSISTENT_WRAP, 2, 1, 0, 100), (lt.FUSED_PERSISTENT_DYNAMIC, 2, 2, 40, 1 << 22),
+                                          (lt.FUSED_PERSISTENT_DYNAMIC, 1, 4, 70, 150), (lt.FUSED_PERSISTENT_STATIC, 2, 4, 0, 1 << 22),
+                                          (lt.FUSED_PERSISTENT_STATIC, 1, 8, 0, 64)):
+            tr.set_option(lt.OPT_FUSED_MODE, mode)
+            tr.set_option(lt.OPT_FUSED_ILP, ilp)
+            tr.set_option(lt.OPT_WARPS_PER_SMSP, w)
+            tr.set_option(lt.OPT_ITEM_TURNS, item)
+            tr.set_option(lt.OPT_CHUNK_TURNS, chunk)
+            out = gpu_programme(tr, z0, d0, a, psi, "fused")
+            assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1]), (split, mode, ilp, w, item, chunk)
+            assert tr.get_stat(lt.STAT_LAST_MODE) == mode and tr.get_stat(lt.STAT_LAST_ILP) == ilp
+
+
 @pytest.mark.parametrize("turns", [1, 2, 31, 32, 33, 64, 65, 97])
 def test_programme_call_lengths_around_the_staging_block(turns):
     """The fused kernel stages the table in blocks of 32 entries per warp and peels the call's
