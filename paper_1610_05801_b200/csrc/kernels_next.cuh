@@ -203,12 +203,7 @@ slice_histogram_kernel(const double* __restrict__ z_arr, size_t n, const __grid_
                        unsigned long long* __restrict__ acc, unsigned int* __restrict__ arrived) {
     extern __shared__ unsigned int slice_smem[];
     __shared__ int is_last;
-    SliceAcc sl;
-    sl.init(X, 0ULL, slice_smem);
-    unsigned long long* const out = sl.out;
-    if (acc) sl.out = acc;
     const size_t head = ((reinterpret_cast<uintptr_t>(z_arr) & 15u) != 0 && n > 0) ? 1 : 0;
-    if (head && blockIdx.x == 0 && threadIdx.x == 0) sl.add(z_arr[0]);
     const double* __restrict__ zb = z_arr + head;
     const size_t m = n - head;
     const size_t tile = (size_t)blockDim.x * 2 * UNR;
@@ -216,11 +211,16 @@ slice_histogram_kernel(const double* __restrict__ z_arr, size_t n, const __grid_
     size_t base = (size_t)blockIdx.x * tile;
     double2 cur[UNR];
     bool have = base + tile <= m;
-    if (have) {
+    if (have) {                               // the first tile is on its way while the counters are zeroed
 #pragma unroll
         for (int u = 0; u < UNR; ++u)
             cur[u] = __ldcs(reinterpret_cast<const double2*>(zb + base) + u * blockDim.x + threadIdx.x);
     }
+    SliceAcc sl;
+    sl.init(X, 0ULL, slice_smem);
+    unsigned long long* const out = sl.out;
+    if (acc) sl.out = acc;
+    if (head && blockIdx.x == 0 && threadIdx.x == 0) sl.add(z_arr[0]);
     while (have) {
         const size_t nb = base + stride;
         const bool more = nb + tile <= m;
