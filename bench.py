@@ -13,7 +13,8 @@ with HOST buffers (lt_track_fused_host: H2D, track, count, D2H inside the timed 
 Everything else the measurement contract asks for sits INSIDE `roofline` (the driver keeps
 that object whole): `per_turn` (configs[3], the HBM-bound half of the metric), `configs`
 (configs[0], [2] and the six configs[4] variants), `f1_chunk_sweep` (turns per launch 1 ..
-2^14 at a fixed total: the B200 redo of the paper's Fig. 5), `next` (the
+2^14 at a fixed total: the B200 redo of the paper's Fig. 5), `size_sweep`
+(n = 2^10 .. 2^24: the analogue of its Table 2), `next` (the
 SURVEY.md sec. 8(f) rows) and `pipe_probe` (what the FP64 pipe issues).  Every leg carries the
 NVML clock record sampled while it ran.  `traffic` values come from profiles/ncu_traffic.json.
 
@@ -328,6 +329,29 @@ def bench_configs(cx: Ctx) -> dict:
                 del z, d, zi, di, tr
     out["clocks"] = clk.summary(short=True)
     return out
+
+
+# ----------------------------------------------------------------------------- particle-count sweep
+def bench_sizes(cx: Ctx) -> dict:
+    """The analogue of the paper's Table 2 (kernel time against the number of
+    macro-particles, flat from 512 to 4096 on 14 SMs): 10^4 leap-frog turns in fused mode for
+    n = 2^10 .. 2^24."""
+    lt, wl = cx.lt, cx.wl
+    turns = 10_000
+    rows = []
+    with cx.clock() as clk:
+        for e in range(10, 25, 2):
+            n = 1 << e
+            z0, d0 = wl.make_bunch(wl.CONFIGS[0], n=n, seed=1000 + e + cx.rank)
+            z, d = cx.dev(z0), cx.dev(d0)
+            tr = lt.Tracker(wl.RING, "leapfrog")
+            sec = cx.timed(lambda: tr.track_fused(z, d, n, turns, cx.sp), 2)
+            rows.append({"n": "2^%d" % e, "ms": round(1e3 * sec, 4), "value": cx.world * n * turns / sec,
+                         "frac": round(FP64_INSTR_PER_PT * n * turns / sec / 1e9 / cx.peak_fp64, 4),
+                         "mode": tr.get_stat(lt.STAT_LAST_MODE), "block": tr.get_stat(lt.STAT_LAST_BLOCK),
+                         "ilp": tr.get_stat(lt.STAT_LAST_ILP)})
+            del z, d, tr
+    return {"turns": turns, "rows": rows, "clocks": clk.summary(short=True)}
 
 
 # ----------------------------------------------------------------------------- f1: chunk-size sweep
@@ -657,6 +681,7 @@ def run_cuda(args) -> None:
     if args.only:                                        # profiling aid: one leg, printed alone
         leg = {"per_turn": bench_per_turn, "configs": bench_configs, "f1": bench_f1,
                "next": bench_next, "probe": lambda c: bench_probe(c, table=True), "shapes": bench_shapes,
+               "sizes": bench_sizes,
                "sharded": bench_per_turn_sharded}.get(args.only)
         if leg is not None:
             res = leg(cx)
@@ -753,6 +778,7 @@ def run_cuda(args) -> None:
     if not args.skip_configs:
         roofline["configs"] = guarded(bench_configs)
         roofline["f1_chunk_sweep"] = guarded(bench_f1)
+        roofline["size_sweep"] = guarded(bench_sizes)
     if not args.skip_next:
         roofline["next"] = guarded(bench_next)
     probe = guarded(bench_probe)
@@ -803,7 +829,7 @@ def main():
     ap.add_argument("--skip-cpu", action="store_true")
     ap.add_argument("--skip-next", action="store_true")
     ap.add_argument("--only", default=None,
-                    choices=["headline", "per_turn", "sharded", "configs", "f1", "next", "probe", "shapes"],
+                    choices=["headline", "per_turn", "sharded", "configs", "f1", "sizes", "next", "probe", "shapes"],
                     help="run one leg alone (for ncu captures and sweeps)")
     args = ap.parse_args()
     if args.impl == "reference":
