@@ -546,8 +546,24 @@ def bench_next(cx: Ctx) -> dict:
         sec = cx.timed(lambda: tr.slice_histogram(zs, n, z_lo, z_hi, S, h1, sp), 8)
         # context for a 12 us operation: the same 80 MB summed by the library reduction, same timer
         ref = cx.timed(lambda: zs.sum(), 8)
+        # the 256 MB fill leaves the L2 full of DIRTY lines, which a read-only 80 MB pass then has to
+        # evict: the same call over five rotating inputs (400 MB > L2, clean lines), back to back
+        rot = [zs] + [zs.clone() for _ in range(4)]
+        for zz in rot:
+            tr.slice_histogram(zz, n, z_lo, z_hi, S, h1, sp)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(cx.stream)
+        for r in range(50):
+            tr.slice_histogram(rot[r % 5], n, z_lo, z_hi, S, h1, sp)
+        e1.record(cx.stream)
+        torch.cuda.synchronize()
+        clean = cx.max_over_ranks(e0.elapsed_time(e1) * 1e-3) / 50
+        del rot
         out["f4_slice_histogram"] = {"n": n, "slices": S, "value": W * n / sec, "unit": "particles/s",
                                      "us_per_call": 1e6 * sec, "us_torch_sum_same_array": 1e6 * ref,
+                                     "us_per_call_rotating_inputs_clean_l2": 1e6 * clean,
+                                     "frac_rotating_inputs_clean_l2": 8 * n / clean / 1e9 / cx.hbm_peak,
                                      "us_in_kernel_ncu": cx.traffic.get("f4_slice_histogram_ncu_us"),
                                      "roofline": cx.hbm(8, n, sec, "f4_slice_histogram")}
         del z, d, zs, hist, mom, tr
