@@ -72,8 +72,11 @@ def ncu_traffic() -> dict:
     committed captures (each entry names its ncu command and the commit it was taken at)."""
     try:
         raw = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
-        return {k: int(v["dram_bytes_read"]) + int(v["dram_bytes_write"])
-                for k, v in raw.get("kernels", {}).items()}
+        out = {k: int(v["dram_bytes_read"]) + int(v["dram_bytes_write"])
+               for k, v in raw.get("kernels", {}).items()}
+        out.update({k + "_ncu_us": float(v["duration_us"]) for k, v in raw.get("kernels", {}).items()
+                    if "duration_us" in v})
+        return out
     except Exception:
         return {}
 
