@@ -379,6 +379,9 @@ int track_fused_persistent(lt_tracker* tr, T* z, T* d, size_t n, unsigned long l
     while (done < turns) {
         unsigned long long chunk = std::min<unsigned long long>(turns - done, (unsigned long long)tr->chunk_turns);
         const int first = done == 0, last = done + chunk == turns;
+        // a launch of a few turns is launch-bound (bench.py's f1 sweep): static slots then,
+        // which need neither the memset of the progress words nor any flag traffic
+        if (pl.dynamic && chunk <= 64 && tr->fused_mode == 0) pl.dynamic = 0;
         const unsigned int item = pl.dynamic == 1 ? std::min<unsigned int>(pl.item_turns, (unsigned int)chunk) : (unsigned int)chunk;
         if (pl.dynamic) {                                    // ticket + progress words of this launch
             LT_CUDA(tr, cudaMemsetAsync(tr->sched, 0, 8 + 4 * ((n + 31) / 32), st));
