@@ -614,11 +614,15 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
 template <typename T>
 __device__ __forceinline__ bool in_bucket(T z, T delta, const MapConsts<T>& P) {
     typedef Real<T> R;
-    T t;
-    T g = reduce_half_periods(R::mul(z, R::mul(P.to_phase, T(0.5))), &t);
+    // |z| < z_max means |g| < 1/2 for g = kappa z / (2 pi): already inside the polynomial's range,
+    // so no range reduction is needed (outside it the value is garbage, and the |z| test is false).
+    // Same bits as with the reduction, 3 FP64 instructions fewer; the r-term only when r != 0
+    // (a warp-uniform branch on a constant): 15 instead of 22 FP64 instructions per particle for
+    // the single harmonic -- the per-turn kernel spends 3.5 us of its 45 on the moments.
+    T g = R::mul(z, R::mul(P.to_phase, T(0.5)));
     T S = R::mul(g, horner<T, R::NS>(P.sin1, R::mul(g, g)));
-    T S2 = R::mul(S, S);
-    T pot = R::mul(S2, R::fma(P.two_r, R::sub(T(1), S2), T(1)));
+    T pot = R::mul(S, S);
+    if (P.two_r != T(0)) pot = R::mul(pot, R::fma(P.two_r, R::sub(T(1), pot), T(1)));
     T hn = R::fma(P.hn_delta, R::mul(delta, delta), pot);
     return (fabs(z) < P.z_max) && (hn < T(1));
 }
