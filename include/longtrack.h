@@ -140,7 +140,8 @@ enum {
     LT_OPT_FUSED_BLOCK    = 4, /* threads per block in fused mode: 0 = planner decides     */
     LT_OPT_PER_TURN_GRAPH = 5, /* 1 (default): per-turn launches are replayed from a CUDA
                                   graph in batches; 0: plain stream launches               */
-    LT_OPT_PER_TURN_CTAS_PER_SM = 6, /* persistent CTAs per SM of the per-turn kernel      */
+    LT_OPT_PER_TURN_CTAS_PER_SM = 6, /* CTAs per SM of the per-turn kernels' grid; 0 (default):
+                                  planner -- 6 up to 1.5e7 particles, 12 beyond; 1..32 forces it */
     LT_OPT_PER_TURN_REVERSE = 7, /* 1 (default): odd turns walk the arrays backwards so the
                                   tail the previous turn left in L2 is read first          */
     LT_OPT_FUSED_MODE     = 8, /* 0 (default): planner picks the persistent kernel's schedule;

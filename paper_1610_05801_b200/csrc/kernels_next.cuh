@@ -19,8 +19,10 @@ namespace lt {
 __device__ __forceinline__ int slice_bin(double z, double z_lo, double z_hi, double inv, int S) {
     if (z < z_lo) return 0;
     if (!(z < z_hi)) return S + 1;
-    const double u = __dmul_rn(__dsub_rn(z, z_lo), inv);   // >= 0: truncation is floor
-    const int s = (int)u;
+    const double u = __dmul_rn(__dsub_rn(z, z_lo), inv);   // 0 <= u < 2^21
+    // floor(u) without a conversion: 2^52 + u rounded toward -inf carries floor(u) in its low
+    // mantissa word, exactly (F2I.F64 runs at a quarter of the FP64 rate; this is one DADD)
+    const int s = __double2loint(__dadd_rd(u, 4503599627370496.0));
     return 1 + (s < S - 1 ? s : S - 1);
 }
 
@@ -192,17 +194,19 @@ static __global__ void advance_cursor_kernel(unsigned long long* cursor, unsigne
 // shared-memory atomics of tile k (128 B per thread; the first version issued a tile's loads only
 // after the previous tile's atomics and ran 1184 short-lived CTAs whose zero / load / flush
 // phases coincided: 3.7 TB/s in the kernel, profiles/r1_next_rows_ncu.md).
-// No memset launch: the CTAs add their counts into a tracker-owned accumulator `acc` that is
-// zero between calls; the last CTA to finish (ticket in *arrived) copies it over the caller's
-// histogram and zeroes it again.  acc == nullptr: the counts go straight into `out`, which the
-// caller zeroed (more slices than the shared-memory path holds).
+// No memset launch and no serial tail: CTA 0 zeroes the caller's histogram while its first tile is
+// in flight and then publishes the call's `epoch` in *flag (release); every CTA streams its
+// share into its shared-memory copies and, ~15 us later, adds them to the caller's histogram
+// after an acquire-read of the flag (CTA 0 is the first CTA the hardware dispatches, so the flag
+// is never actually waited on).  Round 2's first version summed into a tracker-owned accumulator
+// that the LAST CTA copied out: a serial fence + ticket + copy behind the slowest CTA.
+// flag == nullptr: the caller zeroed `out` (more slices than the shared-memory path holds).
 // A z array that is only 8-byte aligned is shifted by one element (`head`).
 template <int UNR>
 static __global__ void __launch_bounds__(512)
 slice_histogram_kernel(const double* __restrict__ z_arr, size_t n, const __grid_constant__ TurnExtras X,
-                       unsigned long long* __restrict__ acc, unsigned int* __restrict__ arrived) {
+                       unsigned int* __restrict__ flag, unsigned int epoch) {
     extern __shared__ unsigned int slice_smem[];
-    __shared__ int is_last;
     const size_t head = ((reinterpret_cast<uintptr_t>(z_arr) & 15u) != 0 && n > 0) ? 1 : 0;
     const double* __restrict__ zb = z_arr + head;
     const size_t m = n - head;
@@ -216,10 +220,14 @@ slice_histogram_kernel(const double* __restrict__ z_arr, size_t n, const __grid_
         for (int u = 0; u < UNR; ++u)
             cur[u] = __ldcs(reinterpret_cast<const double2*>(zb + base) + u * blockDim.x + threadIdx.x);
     }
+    if (flag && blockIdx.x == 0) {
+        for (int b = threadIdx.x; b < X.n_slices + 2; b += blockDim.x) X.hist[b] = 0ULL;
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) st_release_u32(flag, epoch);
+    }
     SliceAcc sl;
     sl.init(X, 0ULL, slice_smem);
-    unsigned long long* const out = sl.out;
-    if (acc) sl.out = acc;
     if (head && blockIdx.x == 0 && threadIdx.x == 0) sl.add(z_arr[0]);
     while (have) {
         const size_t nb = base + stride;
@@ -241,21 +249,13 @@ slice_histogram_kernel(const double* __restrict__ z_arr, size_t n, const __grid_
     for (size_t i = base + threadIdx.x; i < m && base < m; i += blockDim.x) {
         if (i < base + tile) sl.add(zb[i]);
     }
-    sl.flush();
-    if (acc) {
-        __threadfence();
-        __syncthreads();
-        if (threadIdx.x == 0) is_last = atomicAdd(arrived, 1u) == gridDim.x - 1;
-        __syncthreads();
-        if (is_last) {
-            __threadfence();
-            for (int b = threadIdx.x; b < X.n_slices + 2; b += blockDim.x) {
-                out[b] = __ldcg(acc + b);
-                acc[b] = 0ULL;
-            }
-            if (threadIdx.x == 0) *arrived = 0u;
+    if (flag && blockIdx.x != 0) {            // the histogram has been zeroed for THIS call
+        if (threadIdx.x == 0) {
+            while (ld_acquire_u32(flag) != epoch) __nanosleep(32);
         }
+        // SliceAcc::flush starts with a __syncthreads(), which orders every thread behind the acquire
     }
+    sl.flush();
 }
 
 // Programme table of one fused launch, double2 per turn behind a one-entry header:

@@ -461,7 +461,7 @@ int track_transverse_per_turn(lt_tracker* tr, double* x, double* xp, double* y, 
                      (!longi || (aligned(z, 16) && aligned(d, 16)));
     const size_t per_cta = (size_t)kPerTurnThreads * (vec ? 2 : 1);
     size_t g = (n + per_cta - 1) / per_cta;
-    g = std::max<size_t>(1, std::min<size_t>(g, (size_t)tr->sm_count * (size_t)tr->per_turn_ctas_per_sm));
+    g = std::max<size_t>(1, std::min<size_t>(g, (size_t)tr->sm_count * (size_t)(tr->per_turn_ctas_per_sm > 0 ? tr->per_turn_ctas_per_sm : 6)));
     const size_t smem = (size_t)tr->n_seg * 16 * sizeof(double);
     const bool zvec = z && aligned(z, 16) && aligned(d, 16);
     const int zgrid = z ? per_turn_grid(tr, n) : 0;
@@ -547,18 +547,18 @@ int lt_slice_histogram(lt_tracker* tr, const double* z_dev, size_t n, double z_l
         LT_CUDA(tr, cudaMemsetAsync(hist_dev, 0, ((size_t)n_slices + 2) * sizeof(unsigned long long), st));
         if (n == 0) return LT_OK;
     } else if (!tr->hist_acc) {
-        // accumulator of the shared-memory path (<= 8190 slices) + the arrival ticket, zero between calls
-        const size_t bytes = (size_t)(kMaxSharedSlices + 2 + 1) * sizeof(unsigned long long);
-        LT_CUDA(tr, cudaMallocAsync((void**)&tr->hist_acc, bytes, st));
-        LT_CUDA(tr, cudaMemsetAsync(tr->hist_acc, 0, bytes, st));
+        // the epoch flag of the shared-memory path: CTA 0 publishes "the histogram of call number
+        // hist_epoch has been zeroed" in it
+        LT_CUDA(tr, cudaMallocAsync((void**)&tr->hist_acc, sizeof(unsigned long long), st));
+        LT_CUDA(tr, cudaMemsetAsync(tr->hist_acc, 0, sizeof(unsigned long long), st));
     }
     constexpr int kUnr = 4, kThreads = 512;                   // 2 x 64 B in flight per thread
     size_t g = (n + kThreads * 2 * kUnr - 1) / (kThreads * 2 * kUnr);
     g = std::max<size_t>(1, std::min<size_t>(g, (size_t)tr->sm_count * 2));
     const size_t smem = slice_smem_bytes(X);
-    unsigned long long* acc = direct ? nullptr : tr->hist_acc;
+    if (!direct && ++tr->hist_epoch == 0u) tr->hist_epoch = 1u;   // 0 is the flag's initial value
     slice_histogram_kernel<kUnr><<<(unsigned)g, kThreads, smem, st>>>(
-        z_dev, n, X, acc, reinterpret_cast<unsigned int*>(tr->hist_acc ? tr->hist_acc + kMaxSharedSlices + 2 : nullptr));
+        z_dev, n, X, direct ? nullptr : reinterpret_cast<unsigned int*>(tr->hist_acc), tr->hist_epoch);
     LT_CUDA(tr, cudaGetLastError());
     tr->launches++;
     return LT_OK;

@@ -79,8 +79,9 @@ struct lt_tracker {
     // f2: packed programme table of the current fused chunk
     double2* prog_table;
     size_t prog_entries;
-    // f4: accumulator of lt_slice_histogram (kMaxSharedSlices + 2 counters + arrival ticket), zero between calls
+    // f4: epoch flag of lt_slice_histogram ("the caller's histogram has been zeroed for call hist_epoch")
     unsigned long long* hist_acc;
+    unsigned int hist_epoch;
     // f2 with acceleration: packed sub-step entries (lt::RampEntry, 48 B each)
     void* ramp_table;
     size_t ramp_entries;

@@ -88,7 +88,7 @@ def test_options_and_stats(lt):
     tr.set_option(lt.OPT_CHUNK_TURNS, 1000)
     assert tr.get_option(lt.OPT_CHUNK_TURNS) == 1000
     for opt, bad in ((lt.OPT_CHUNK_TURNS, 0), (lt.OPT_FUSED_ILP, 3), (lt.OPT_FUSED_BLOCK, 100),
-                     (lt.OPT_PER_TURN_CTAS_PER_SM, 0), (lt.OPT_FUSED_MODE, 5),
+                     (lt.OPT_PER_TURN_CTAS_PER_SM, -1), (lt.OPT_PER_TURN_CTAS_PER_SM, 33), (lt.OPT_FUSED_MODE, 5),
                      (lt.OPT_WARPS_PER_SMSP, 9), (lt.OPT_FLIP_ON_Q, 2), (99, 1)):
         with pytest.raises(lt.LongtrackError) as e:
             tr.set_option(opt, bad)
