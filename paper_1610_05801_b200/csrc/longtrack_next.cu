@@ -554,8 +554,10 @@ int lt_slice_histogram(lt_tracker* tr, const double* z_dev, size_t n, double z_l
     }
     constexpr int kUnr = 4, kThreads = 512;                   // 2 x 64 B in flight per thread
     size_t g = (n + kThreads * 2 * kUnr - 1) / (kThreads * 2 * kUnr);
-    g = std::max<size_t>(1, std::min<size_t>(g, (size_t)tr->sm_count * 2));
     const size_t smem = slice_smem_bytes(X);
+    // one wave: as many CTAs as are resident together (the flag protocol of the kernel needs CTA 0
+    // running while the others wait for it; it is the first one dispatched)
+    g = std::max<size_t>(1, std::min<size_t>(g, (size_t)tr->sm_count * 2));   // 3 per SM measured the same
     if (!direct && ++tr->hist_epoch == 0u) tr->hist_epoch = 1u;   // 0 is the flag's initial value
     slice_histogram_kernel<kUnr><<<(unsigned)g, kThreads, smem, st>>>(
         z_dev, n, X, direct ? nullptr : reinterpret_cast<unsigned int*>(tr->hist_acc), tr->hist_epoch);

@@ -263,6 +263,38 @@ def test_slice_histogram_sizes_around_a_tile_and_8_byte_alignment(n, offset):
                           oracle.slice_histogram(z[offset:], -0.7, 0.7, 64))
 
 
+def test_slice_index_is_branch_free_but_exact_on_special_values():
+    """The slice index is computed without branches (floor through a magic-number add, selects
+    for the two overflow bins): signed zeros at z_lo = 0, values whose scaled offset overflows
+    32 bits in either direction, denormals, infinities and NaN must land where G29 puts them."""
+    tr, _ = both()
+    big = [1e300, -1e300, 3e9, -3e9, 2.0 ** 31, -2.0 ** 31, 2.0 ** 52, -2.0 ** 52, 5e-324, -5e-324,
+           0.0, -0.0, np.inf, -np.inf, np.nan, 1.0, np.nextafter(1.0, 0), np.nextafter(0.0, 1)]
+    z = np.array(big * 3 + [0.25, 0.5, 0.75], dtype=np.float64)
+    for z_lo, z_hi, S in ((0.0, 1.0, 4), (-0.0, 1.0, 4), (-1.0, 0.0, 3), (0.0, 1e-300, 5), (-1e300, 1e300, 7),
+                          (0.0, 1.0, 1 << 20)):
+        assert np.array_equal(gpu_hist(tr, z, z_lo, z_hi, S), oracle.slice_histogram(z, z_lo, z_hi, S)), (z_lo, z_hi, S)
+
+
+def test_slice_histogram_repeated_calls_on_one_tracker():
+    """Every call zeroes the caller's histogram itself (CTA 0 publishes an epoch the other CTAs
+    wait for): back-to-back calls of one tracker into different and into the same output, with
+    sizes on both sides of one wave of CTAs, never see each other's counts."""
+    tr, _ = both()
+    rng = np.random.default_rng(5)
+    outs = []
+    for k, n in enumerate((3, 700_001, 5, 1_300_000, 1_300_000, 64)):
+        z = rng.normal(0.0, 0.3, n)
+        zt = dev(z)
+        h = torch.full((64 + 2,), 12345, dtype=torch.int64, device="cuda")
+        for _ in range(3 if k == 4 else 1):                # the same output three times in a row
+            tr.slice_histogram(zt, n, -0.7, 0.7, 64, h, stream_ptr())
+        outs.append((h, oracle.slice_histogram(z, -0.7, 0.7, 64), zt))
+    torch.cuda.synchronize()
+    for h, ho, _ in outs:
+        assert np.array_equal(h.cpu().numpy().astype(np.uint64), ho)
+
+
 def test_slice_edges_on_a_dyadic_grid_and_empty_input():
     tr, _ = both()
     S = 8
