@@ -136,7 +136,9 @@ enum {
                                   of one call does not depend on it     */
     LT_OPT_FUSED_ILP      = 3, /* particles per lane in fused mode: 0 = planner decides; 1, 2 for
                                   the persistent kernels (fp32: PAIRS of particles per lane, the
-                                  arithmetic is packed two to a value), 1, 2, 4 for the plain one  */
+                                  arithmetic is packed two to a value), 1, 2, 4 for the plain one,
+                                  1, 2, 4, 8 for the fused transverse kernel (other kernels read 8
+                                  as 0)                                                            */
     LT_OPT_FUSED_BLOCK    = 4, /* threads per block in fused mode: 0 = planner decides     */
     LT_OPT_PER_TURN_GRAPH = 5, /* 1 (default): per-turn launches are replayed from a CUDA
                                   graph in batches; 0: plain stream launches               */

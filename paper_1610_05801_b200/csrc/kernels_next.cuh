@@ -357,7 +357,7 @@ __device__ __forceinline__ void transverse_turn(double (&u)[ILP][4], unsigned in
 // Particle j of a lane is element  g*32*ILP + j*32 + lane  (coalesced).  The arithmetic per
 // particle does not depend on ILP, so every launch shape returns the same bits.
 template <int NSEG, bool LONGI, int ILP>
-__global__ void __launch_bounds__(ILP == 1 ? 1024 : 512, 1)
+__global__ void __launch_bounds__(ILP == 1 ? 1024 : (ILP == 8 ? 256 : 512), 1)
 transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp_arr,
                              double* __restrict__ y_arr, double* __restrict__ yp_arr,
                              double* __restrict__ z_arr, double* __restrict__ d_arr, size_t n,

@@ -152,7 +152,7 @@ FusedPlan plan_fused(const lt_tracker* tr, size_t n) {
     for (int b : blocks) {
         if (tr->fused_block > 0 && b != tr->fused_block) continue;
         for (int ilp : ilps) {
-            if (tr->fused_ilp > 0 && ilp != tr->fused_ilp) continue;
+            if (tr->fused_ilp > 0 && tr->fused_ilp <= 4 && ilp != tr->fused_ilp) continue;   // 8: transverse kernel only
             const long long tile = (long long)b * ilp;
             const long long grid = (long long)((n + tile - 1) / tile);
             const int max_res = std::min(32, 2048 / b);           // resident CTAs per SM
@@ -721,7 +721,7 @@ int lt_set_option(lt_tracker* tr, int option, long long value) {
             if (value < 1 || value > (1LL << 31) - 1) return LT_E_PARAM;
             tr->chunk_turns = value; return LT_OK;
         case LT_OPT_FUSED_ILP:
-            if (value != 0 && value != 1 && value != 2 && value != 4) return LT_E_PARAM;
+            if (value != 0 && value != 1 && value != 2 && value != 4 && value != 8) return LT_E_PARAM;
             tr->fused_ilp = value; return LT_OK;
         case LT_OPT_FUSED_BLOCK:
             if (value != 0 && value != 32 && value != 64 && value != 128) return LT_E_PARAM;

@@ -304,9 +304,11 @@ int ensure_lattice(lt_tracker* tr, cudaStream_t st) {
     return LT_OK;
 }
 
-// launch shape of the fused transverse kernel: ILP particles per thread (4 or 2 at 4 warps per
-// sub-partition, 128 registers per thread; 1 at the plan of the longitudinal kernel), the largest
-// ILP that still fills one wave of warps; dynamic chunk scheduling beyond one wave
+// launch shape of the fused transverse kernel: ILP particles per thread (8 at 2 warps per
+// sub-partition and 220 registers per thread -- a matrix row fetched from shared memory then feeds
+// 32 FP64 instructions: 0.893 of the FP64 peak against 0.882 with 4 --, 4 or 2 at 4 warps per
+// sub-partition and 128 registers; 1 at the plan of the longitudinal kernel), the largest ILP
+// that still fills one wave of warps; dynamic chunk scheduling beyond one wave
 struct TransPlan { int ilp; PersistentPlan pl; };
 
 TransPlan plan_transverse(const lt_tracker* tr, size_t n, unsigned long long turns) {
@@ -314,7 +316,8 @@ TransPlan plan_transverse(const lt_tracker* tr, size_t n, unsigned long long tur
     tp.ilp = 1;
     const unsigned long long slots = (unsigned long long)tr->sm_count * 16;
     int ilp = 0;
-    if (tr->fused_ilp == 1 || tr->fused_ilp == 2 || tr->fused_ilp == 4) ilp = (int)tr->fused_ilp;
+    if (tr->fused_ilp == 1 || tr->fused_ilp == 2 || tr->fused_ilp == 4 || tr->fused_ilp == 8) ilp = (int)tr->fused_ilp;
+    else if ((n + 255) / 256 >= slots / 2) ilp = 8;
     else if ((n + 127) / 128 >= slots) ilp = 4;
     else if ((n + 63) / 64 >= slots) ilp = 2;
     else ilp = 1;
@@ -332,10 +335,12 @@ TransPlan plan_transverse(const lt_tracker* tr, size_t n, unsigned long long tur
     tp.ilp = ilp;
     const unsigned long long groups = (n + 32 * ilp - 1) / (32 * ilp);
     PersistentPlan pl = {0, 4, 1, 512, 0, true, 1};
+    if (ilp == 8) { pl.warps_per_smsp = 2; pl.threads = 256; }   // 220 registers per thread
     // more groups than slots: the ticket queue (4 warps per sub-partition hide its item switches; the
     // wrap-around static schedule measured 1.2 points lower and its code cost the kernel a register
     // spill, so this kernel does not carry it: LT_OPT_FUSED_MODE = 4 means the queue here)
-    pl.dynamic = tr->fused_mode == 2 ? 0 : ((groups > slots || tr->fused_mode >= 3) ? 1 : 0);
+    const unsigned long long my_slots = ilp == 8 ? slots / 2 : slots;
+    pl.dynamic = tr->fused_mode == 2 ? 0 : ((groups > my_slots || tr->fused_mode >= 3) ? 1 : 0);
     if (pl.dynamic == 1) {
         unsigned long long it = tr->item_turns > 0
                                     ? (unsigned long long)tr->item_turns
@@ -383,6 +388,7 @@ template <bool LONGI>
 cudaError_t launch_transverse(double* x, double* xp, double* y, double* yp, double* z, double* d,
                               size_t n, unsigned int turns, unsigned int item_turns, int first, int last,
                               const TransPlan& tp, const lt_tracker* tr, cudaStream_t st) {
+    if (tp.ilp == 8) return launch_transverse_ilp<LONGI, 8>(x, xp, y, yp, z, d, n, turns, item_turns, first, last, tp.pl, tr, st);
     if (tp.ilp == 4) return launch_transverse_ilp<LONGI, 4>(x, xp, y, yp, z, d, n, turns, item_turns, first, last, tp.pl, tr, st);
     if (tp.ilp == 2) return launch_transverse_ilp<LONGI, 2>(x, xp, y, yp, z, d, n, turns, item_turns, first, last, tp.pl, tr, st);
     return launch_transverse_ilp<LONGI, 1>(x, xp, y, yp, z, d, n, turns, item_turns, first, last, tp.pl, tr, st);
