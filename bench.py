@@ -52,7 +52,7 @@ FP32_INSTR = {("leapfrog", 0.0): 10, ("euler_cromer", 0.0): 10, ("ruth4", 0.0): 
               ("leapfrog", 0.5): 17, ("euler_cromer", 0.5): 17, ("ruth4", 0.5): 51}
 FP64_INSTR_PER_PT = FP64_INSTR[("leapfrog", 0.0)]
 INSTR_F2_PROGRAMME = 15                   # 13 + f*a_t + the phase-offset add
-INSTR_F2_RAMP = 16                        # 13 + f*(g amp) + (g delta + c) + the phase-offset add
+INSTR_F2_RAMP = 15                        # 13 + (G y + C) + the phase-offset add (scaled layout; 16 with f*(g amp) in the plain one)
 BYTES_PER_PT_PER_TURN_MODE = 32           # 16 B read + 16 B write per particle-turn
 SMS, FP64_LANES_PER_SM, FP32_LANES_PER_SM = 148, 64, 128
 CPU_SAMPLE_TURNS = 10_000                 # all-cores oracle leg: 1e9 particle-turns

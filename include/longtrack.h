@@ -158,8 +158,13 @@ enum {
     LT_OPT_WARPS_PER_SMSP = 10,/* resident warps per SM sub-partition of the persistent kernel
                                   (0 = planner; 1..8, or even values up to 16; with two particles
                                   per lane at most 4)                                               */
-    LT_OPT_FLIP_ON_Q      = 11 /* where the sign of the reduced sine is applied: -1 planner,
+    LT_OPT_FLIP_ON_Q      = 11,/* where the sign of the reduced sine is applied: -1 planner,
                                   0 on the argument, 1 on the polynomial; same bits either way */
+    LT_OPT_RAMP_SCALED    = 12 /* lt_track_ramp, merged drifts: 1 (default) carries delta divided by
+                                  the running kick amplitude (15 FP64 instructions per sub-step,
+                                  four table values) whenever no voltage scale of the call is zero;
+                                  0 always the plain form (16 instructions, five values).  The two
+                                  round differently (both far inside the 1e-9 gate).              */
 };
 
 /* Counters for lt_get_stat. */

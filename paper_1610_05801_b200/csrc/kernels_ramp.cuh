@@ -35,6 +35,21 @@ struct RampEntry {
     double d0, d1;
 };
 
+// SCALED fast layout (round 2): the fused kernel carries  y = delta / lambda_K  instead of delta,
+// with lambda_0 = 1 and lambda_(K+1) = g_K amp_K, the scale in effect after sub-step K.  Then
+//     y' = (lambda_K / amp_K) y + c_K / lambda_(K+1) + [sin(pi u) + r sin(2 pi u)]
+// -- the kick amplitude has left the kick: no f * ga multiply, FOUR table values per sub-step
+// instead of five (two 16-byte shared-memory loads instead of three), 15 FP64 instructions
+// instead of 16.  The drift coefficient carries the scale: u' = (u + dp) - (d0 lambda_(K+1)) y'.
+// Needs amp_K != 0 for every sub-step of the call: a scan of the voltage table decides per CALL
+// between this layout and the plain fast layout above (ramp_scan_kernel, *flag != 0: plain).
+// Header entry: dp = absolute psi/pi of the launch's first sub-step, C = lambda after the
+// launch's LAST sub-step (delta = y * C at the end of a call), D = leading drift of the call.
+struct RampScaled {
+    double G, dp;       // lambda_K / amp_K;  RF phase offset difference to the next sub-step (half periods)
+    double C, D;        // c_K / lambda_(K+1);  merged drift coefficient times lambda_(K+1)
+};
+
 struct RampRing {
     double mc2, alpha_c, qV, C;   // rest energy (eV), momentum compaction, q V (eV), circumference
     double x1, x0;                // Ruth4 step factors
@@ -50,14 +65,49 @@ __device__ __forceinline__ void ramp_ring_at(const RampRing& R, double p, double
     *d = eta * R.C * 0.5;
 }
 
+// Momenta, kick amplitudes and drift coefficients of the sub-steps of ONE turn (reference
+// pb -> pa, voltage scale av): ps[0..nsub], A[..], d[..] at those momenta, tau[0..nsub-1].
+struct RampTurn { double ps[4], A[4], d[4], tau[3]; int nsub; };
+__device__ __forceinline__ void ramp_turn_at(const RampRing& R, double pb, double pa, int integ, RampTurn* t) {
+    t->nsub = integ == kRuth4 ? 3 : 1;
+    t->ps[0] = pb;
+    if (t->nsub == 3) {
+        const double D = pa - pb;
+        t->ps[1] = __fma_rn(R.x1, D, pb);
+        t->ps[2] = __fma_rn(R.x0, D, t->ps[1]);
+        t->ps[3] = pa;
+        t->tau[0] = R.x1; t->tau[1] = R.x0; t->tau[2] = R.x1;
+    } else {
+        t->ps[1] = pa;
+        t->tau[0] = 1.0; t->tau[1] = 0.0; t->tau[2] = 0.0;
+    }
+    for (int k = 0; k <= t->nsub; ++k) ramp_ring_at(R, t->ps[k], &t->A[k], &t->d[k]);
+}
+// g = p_b/p_a and g * amp of sub-step k (the scale lambda in effect after it)
+__device__ __forceinline__ double ramp_g(const RampTurn& t, int k) { return t.ps[k] / t.ps[k + 1]; }
+__device__ __forceinline__ double ramp_ga(const RampTurn& t, int k, double av) {
+    return ramp_g(t, k) * (t.tau[k] * t.A[k] * av);
+}
+
+// *flag |= 1 when any voltage scale of the call is zero (the scaled layout divides by the kick amplitude)
+static __global__ void ramp_scan_kernel(const double* __restrict__ volt, unsigned long long turns,
+                                        unsigned int* __restrict__ flag) {
+    bool zero = false;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < turns;
+         i += (unsigned long long)gridDim.x * blockDim.x)
+        zero |= !(fabs(volt[i]) > 0.0);                        // zero or NaN
+    if (__syncthreads_or(zero) && threadIdx.x == 0) atomicOr(flag, 1u);
+}
+
 // One thread per turn of the launch.  p0c / volt / phase are the CALL's tables (volt, phase may be
 // nullptr), t_first the absolute index of the launch's first turn, call_turns the call's length
 // (the trailing drift of the call's last sub-step is not merged with anything).
+// fast = 1: the plain fast layout into `out`; and, when out2 != nullptr, the scaled layout into out2.
 static __global__ void ramp_pack_kernel(const double* __restrict__ p0c, const double* __restrict__ volt,
                                  const double* __restrict__ phase, unsigned long long t_first,
                                  unsigned int count, unsigned long long call_turns, int integ,
                                  int fast, const __grid_constant__ RampRing R,
-                                 RampEntry* __restrict__ out) {
+                                 RampEntry* __restrict__ out, RampScaled* __restrict__ out2) {
     const unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= count) return;
     const unsigned long long T = t_first + i;
@@ -65,21 +115,10 @@ static __global__ void ramp_pack_kernel(const double* __restrict__ p0c, const do
     const double av = volt ? volt[T] : 1.0;
     const double psi = phase ? phase[T] : 0.0;
     const double psi_next = (phase && T + 1 < call_turns) ? phase[T + 1] : 0.0;
-    const int nsub = integ == kRuth4 ? 3 : 1;
-    double ps[4], tau[3];
-    ps[0] = pb;
-    if (nsub == 3) {
-        const double D = pa - pb;
-        ps[1] = __fma_rn(R.x1, D, pb);
-        ps[2] = __fma_rn(R.x0, D, ps[1]);
-        ps[3] = pa;
-        tau[0] = R.x1; tau[1] = R.x0; tau[2] = R.x1;
-    } else {
-        ps[1] = pa;
-        tau[0] = 1.0;
-    }
-    double A[4], d[4];
-    for (int k = 0; k <= nsub; ++k) ramp_ring_at(R, ps[k], &A[k], &d[k]);
+    RampTurn t;
+    ramp_turn_at(R, pb, pa, integ, &t);
+    const int nsub = t.nsub;
+    const double* ps = t.ps; const double* A = t.A; const double* d = t.d; const double* tau = t.tau;
     const double tau_first = integ == kEulerCromer ? 0.0 : tau[0];
     const double p_here = __dmul_rn(psi, R.inv_pi);
     RampEntry* dst = out + (fast ? 1 : 0);                 // fast layout: behind the header entry
@@ -88,10 +127,18 @@ static __global__ void ramp_pack_kernel(const double* __restrict__ p0c, const do
         h.ga = 0.0; h.p = p_here; h.g = 1.0; h.c = 0.0; h.d0 = 0.0; h.d1 = 0.0;
         out[0] = h;
     }
+    // scaled layout: the scale in effect before this turn's first sub-step is the one the previous
+    // turn's last sub-step left (recomputed here with the same function: the same bits)
+    double lam = 1.0;
+    if (fast && out2 && T > 0) {
+        RampTurn prev;
+        ramp_turn_at(R, p0c[T - 1], pb, integ, &prev);
+        lam = ramp_ga(prev, prev.nsub - 1, volt ? volt[T - 1] : 1.0);
+    }
     for (int k = 0; k < nsub; ++k) {
         RampEntry e;
-        e.g = ps[k] / ps[k + 1];
-        e.ga = e.g * (tau[k] * A[k] * av);
+        e.g = ramp_g(t, k);
+        e.ga = ramp_ga(t, k, av);
         e.p = p_here;
         e.c = -(ps[k + 1] - ps[k]) / ps[k + 1];
         double db = tau[k] * d[k], da = tau[k] * d[k + 1];
@@ -104,12 +151,25 @@ static __global__ void ramp_pack_kernel(const double* __restrict__ p0c, const do
             e.d1 = db * R.to_phase;
             // every sub-step of a turn sees the same psi: the offset changes behind the last one
             e.p = (k + 1 < nsub) ? 0.0 : __dsub_rn(__dmul_rn(psi_next, R.inv_pi), p_here);
+            if (out2) {
+                RampScaled q;
+                const double amp = tau[k] * A[k] * av;
+                const double lam_next = e.ga;              // g_K amp_K
+                q.G = lam / amp;
+                q.dp = e.p;
+                q.C = e.c / lam_next;
+                q.D = e.d0 * lam_next;
+                out2[1 + (size_t)i * nsub + k] = q;
+                if (i == 0 && k == 0) { out2[0].G = 0.0; out2[0].dp = p_here; out2[0].D = e.d1; }
+                lam = lam_next;
+            }
         } else {
             e.d0 = db;
             e.d1 = da;
         }
         dst[(size_t)i * nsub + k] = e;
     }
+    if (fast && out2 && i == count - 1) out2[0].C = lam;   // the scale the launch leaves: delta = y * lam
 }
 
 static __global__ void ramp_advance_cursor_kernel(unsigned long long* cursor, unsigned long long by) {
@@ -158,6 +218,26 @@ __device__ __forceinline__ void ramp_substep_fast(double& u, double& dl, const M
     u = __fma_rn(-dm, dl, w);
 }
 
+// scaled fast sub-step (RampScaled): state (u, y = delta / lambda_K); 15 FP64 instructions (single
+// harmonic): u + dp, 3 reduction, f^2, G y + C, 7 Horner, the kick FMA, the drift FMA
+template <int HARM>
+__device__ __forceinline__ void ramp_substep_scaled(double& u, double& y, const MapConsts<double>& P,
+                                                    double G, double dp, double C, double D) {
+    typedef Real<double> R;
+    const double w = __dadd_rn(u, dp);
+    double t;
+    const double f = reduce_half_periods(u, &t);
+    const double s = __dmul_rn(f, f);
+    const double base = __fma_rn(G, y, C);
+    double q = horner<double, R::NS>(P.sin1, s);
+    if (HARM == 2) {
+        const double cc = horner<double, R::NC>(P.cos1, s);
+        q = __dmul_rn(q, __fma_rn(R::flip_by(P.two_r, t), cc, 1.0));
+    }
+    y = __fma_rn(R::flip(f, t), q, base);
+    u = __fma_rn(-D, y, w);
+}
+
 __device__ __forceinline__ void cp_async_16(void* smem_dst, const void* gmem_src) {
     const unsigned int dst = (unsigned int)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(gmem_src) : "memory");
@@ -166,33 +246,39 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 
 // `nsteps` sub-steps of the ILP particles of a lane; tab = the item's first entry as
-// double2[3 * nsteps]; stage = the warp's private double buffer in shared memory (2 x 32 entries =
-// 3072 B).  While the warp works through one block of 32 entries, the next block arrives by
+// double2[E * nsteps] (E = 3 double2 per entry: RampEntry; E = 2, SCALED: RampScaled); stage = the
+// warp's private double buffer in shared memory (2 x 32 entries = 3072 B / 2048 B).  While the warp
+// works through one block of 32 entries, the next block arrives by
 // cp.async (no registers held, no L2 latency on the dependent FP64 chain; a per-sub-step global
 // load stalled the RF-programme kernel once per 128-byte line, profiles/r1_next_rows_ncu.md).
-template <int HARM, bool SPLIT, int ILP>
+// hdr = the launch's header entry (SCALED: leading drift, absolute offset, final scale).
+template <int HARM, bool SPLIT, int ILP, bool SCALED>
 __device__ __forceinline__ void ramp_advance(double (&x)[ILP], double (&dl)[ILP], unsigned int nsteps,
                                              int first, int last, const MapConsts<double>& P,
                                              const double2* __restrict__ tab,
+                                             const double2* __restrict__ hdr,
                                              double2* __restrict__ stage) {
+    constexpr unsigned int E = SCALED ? 2u : 3u;
     const unsigned int lane = threadIdx.x & 31u;
-    const unsigned int total2 = 3u * nsteps;
+    const unsigned int total2 = E * nsteps;
     auto fetch = [&](unsigned int t0, unsigned int buf) {
 #pragma unroll
-        for (int j = 0; j < 3; ++j) {
-            const unsigned int idx = 3u * t0 + lane + 32u * j;
-            if (idx < total2) cp_async_16(stage + 96u * buf + lane + 32u * j, tab + idx);
+        for (int j = 0; j < (int)E; ++j) {
+            const unsigned int idx = E * t0 + lane + 32u * j;
+            if (idx < total2) cp_async_16(stage + 32u * E * buf + lane + 32u * j, tab + idx);
         }
         cp_async_commit();
     };
     fetch(0, 0);
     if (!SPLIT && first) {
-        const double lead = __ldg(tab + 2).y, p0 = __ldg(tab - 3).y;   // header entry: absolute offset
+        // header entry: absolute offset; leading drift of the call's first sub-step
+        const double lead = SCALED ? __ldg(hdr + 1).y : __ldg(tab + 2).y;
+        const double p0 = __ldg(hdr).y;
 #pragma unroll
         for (int j = 0; j < ILP; ++j) {
             x[j] = __dmul_rn(x[j], P.to_phase);
             x[j] = __fma_rn(-lead, dl[j], x[j]);
-            x[j] = __dadd_rn(x[j], p0);
+            x[j] = __dadd_rn(x[j], p0);                 // SCALED: lambda_0 = 1, y = delta
         }
     }
     unsigned int buf = 0;
@@ -200,38 +286,56 @@ __device__ __forceinline__ void ramp_advance(double (&x)[ILP], double (&dl)[ILP]
         fetch(t0 + 32u, buf ^ 1u);           // the block after this one (an empty group at the end)
         cp_async_wait_1();                   // this block has landed
         __syncwarp();
-        const double2* __restrict__ cur = stage + 96u * buf;
+        const double2* __restrict__ cur = stage + 32u * E * buf;
         const unsigned int m = min(32u, nsteps - t0);
         // the whole staged block unrolled: LDS addresses become immediates and the loop's counter and
         // uniform-register reloads disappear (unroll 4 -> 32: 77.8 % -> 83.3 % of the FP64 peak)
         constexpr int kUnrollR = 32;
 #pragma unroll kUnrollR
         for (unsigned int k = 0; k < m; ++k) {
-            const double2 e0 = cur[3 * k], e1 = cur[3 * k + 1], e2 = cur[3 * k + 2];
+            if (SCALED) {
+                const double2 e0 = cur[2 * k], e1 = cur[2 * k + 1];
 #pragma unroll
-            for (int j = 0; j < ILP; ++j) {
-                if (SPLIT) ramp_substep_exact<HARM>(x[j], dl[j], P, e0.x, e0.y, e1.x, e1.y, e2.x, e2.y);
-                else ramp_substep_fast<HARM>(x[j], dl[j], P, e0.x, e0.y, e1.x, e1.y, e2.x);
+                for (int j = 0; j < ILP; ++j) ramp_substep_scaled<HARM>(x[j], dl[j], P, e0.x, e0.y, e1.x, e1.y);
+            } else {
+                const double2 e0 = cur[3 * k], e1 = cur[3 * k + 1], e2 = cur[3 * k + 2];
+#pragma unroll
+                for (int j = 0; j < ILP; ++j) {
+                    if (SPLIT) ramp_substep_exact<HARM>(x[j], dl[j], P, e0.x, e0.y, e1.x, e1.y, e2.x, e2.y);
+                    else ramp_substep_fast<HARM>(x[j], dl[j], P, e0.x, e0.y, e1.x, e1.y, e2.x);
+                }
             }
         }
         __syncwarp();                        // all lanes are done with `buf` before it is refilled
     }
     if (!SPLIT && last) {
+        const double lam = SCALED ? __ldg(hdr + 1).x : 1.0;
 #pragma unroll
-        for (int j = 0; j < ILP; ++j) x[j] = __dmul_rn(x[j], P.from_phase);
+        for (int j = 0; j < ILP; ++j) {
+            x[j] = __dmul_rn(x[j], P.from_phase);
+            if (SCALED) dl[j] = __dmul_rn(dl[j], lam);
+        }
     }
 }
 
 // Fused multi-turn kernel with the ramp: the persistent ticketed work queue of
 // fused_persistent_kernel (kernels.cuh), work item = (chunk of item_steps sub-steps) x (32 particles).
-template <int HARM, bool SPLIT, int ILP>
+// table = the launch's table INCLUDING its header entry (SPLIT: no header).  SCALED: RampScaled
+// entries.  flag (may be nullptr) = the per-call choice between the two fast layouts, written by
+// ramp_scan_kernel: the SCALED instantiation runs when *flag == 0, the plain one when *flag != 0;
+// the other launch of the pair returns at once.
+template <int HARM, bool SPLIT, int ILP, bool SCALED = false>
 __global__ void __launch_bounds__(ILP == 1 ? 1024 : 512, 1)
 ramp_persistent_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, size_t n,
                        unsigned int nsteps, unsigned int item_steps, int first_launch, int last_launch,
                        int dynamic, unsigned long long* __restrict__ ticket,
                        unsigned int* __restrict__ done, const __grid_constant__ MapConsts<double> P,
-                       const double2* __restrict__ table) {
+                       const double2* __restrict__ table_hdr, const unsigned int* __restrict__ flag) {
     extern __shared__ __align__(16) unsigned char ramp_smem[];   // 3072 B per warp + residency cap
+    static_assert(!(SCALED && SPLIT), "the scaled layout is a fast-path layout");
+    if (flag && ((*flag != 0u) == SCALED)) return;
+    constexpr unsigned int E = SCALED ? 2u : 3u;
+    const double2* __restrict__ table = table_hdr + (SPLIT ? 0u : E);
     constexpr unsigned int G = 32u * ILP;
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned long long groups = (n + G - 1) / G;
@@ -255,7 +359,7 @@ ramp_persistent_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, s
         }
         const int first = first_launch && s_begin == 0;
         const int last = last_launch && s_begin + ns == nsteps;
-        ramp_advance<HARM, SPLIT, ILP>(x, dl, ns, first, last, P, table + 3 * (size_t)s_begin, stage);
+        ramp_advance<HARM, SPLIT, ILP, SCALED>(x, dl, ns, first, last, P, table + E * (size_t)s_begin, table_hdr, stage);
 #pragma unroll
         for (int j = 0; j < ILP; ++j) {
             const size_t i = i0 + 32u * j;

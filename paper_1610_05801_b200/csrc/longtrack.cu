@@ -685,6 +685,7 @@ int lt_create(const lt_params* p, lt_tracker** out) {
     tr->item_turns = 0;
     tr->warps_per_smsp = 0;
     tr->flip_on_q = -1;
+    tr->ramp_scaled = 1;
     *out = tr;
     return LT_OK;
 }
@@ -743,6 +744,7 @@ int lt_set_option(lt_tracker* tr, int option, long long value) {
         case LT_OPT_FLIP_ON_Q:
             if (value < -1 || value > 1) return LT_E_PARAM;
             tr->flip_on_q = value; return LT_OK;
+        case LT_OPT_RAMP_SCALED: tr->ramp_scaled = value != 0; return LT_OK;
         default: return LT_E_PARAM;
     }
 }
@@ -761,6 +763,7 @@ int lt_get_option(const lt_tracker* tr, int option, long long* value) {
         case LT_OPT_ITEM_TURNS: *value = tr->item_turns; return LT_OK;
         case LT_OPT_WARPS_PER_SMSP: *value = tr->warps_per_smsp; return LT_OK;
         case LT_OPT_FLIP_ON_Q: *value = tr->flip_on_q; return LT_OK;
+        case LT_OPT_RAMP_SCALED: *value = tr->ramp_scaled; return LT_OK;
         default: return LT_E_PARAM;
     }
 }

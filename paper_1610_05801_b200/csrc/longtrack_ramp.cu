@@ -34,11 +34,19 @@ RampRing make_ring(const lt_tracker* tr) {
     return R;
 }
 
+// One buffer: `cap` RampEntry (48 B), then `cap` RampScaled (32 B), then the layout flag of the call.
+constexpr size_t kRampBytesPerEntry = sizeof(RampEntry) + sizeof(RampScaled);
 int ensure_ramp_table(lt_tracker* tr, size_t entries, cudaStream_t st) {
-    size_t have = tr->ramp_entries * sizeof(RampEntry);
-    LT_CUDA(tr, grow_async(&tr->ramp_table, &have, entries * sizeof(RampEntry), st));
+    size_t have = tr->ramp_entries ? tr->ramp_entries * kRampBytesPerEntry + 8 : 0;
+    LT_CUDA(tr, grow_async(&tr->ramp_table, &have, entries * kRampBytesPerEntry + 8, st));
     if (tr->ramp_entries < entries) tr->ramp_entries = entries;
     return LT_OK;
+}
+RampScaled* scaled_table(const lt_tracker* tr) {
+    return reinterpret_cast<RampScaled*>(reinterpret_cast<char*>(tr->ramp_table) + tr->ramp_entries * sizeof(RampEntry));
+}
+unsigned int* layout_flag(const lt_tracker* tr) {
+    return reinterpret_cast<unsigned int*>(reinterpret_cast<char*>(tr->ramp_table) + tr->ramp_entries * kRampBytesPerEntry);
 }
 
 int check_args(const lt_tracker* tr, const double* z, const double* d, size_t n,
@@ -53,11 +61,12 @@ int check_args(const lt_tracker* tr, const double* z, const double* d, size_t n,
     return LT_OK;
 }
 
-template <int HARM, bool SPLIT, int ILP>
+// SCALED: the scaled fast layout; flag: the call's layout choice on the device, or nullptr = run
+template <int HARM, bool SPLIT, int ILP, bool SCALED>
 cudaError_t launch_ramp_fused_ilp(double* z, double* d, size_t n, unsigned int nsteps, unsigned int item_steps,
                                   int first, int last, const PersistentPlan& pl, const lt_tracker* tr,
-                                  cudaStream_t st) {
-    auto kern = ramp_persistent_kernel<HARM, SPLIT, ILP>;
+                                  const unsigned int* flag, cudaStream_t st) {
+    auto kern = ramp_persistent_kernel<HARM, SPLIT, ILP, SCALED>;
     // the request caps the CTAs per SM (1 CTA/SM: > half of the 227 KB; 2 CTAs/SM: > a third) and
     // holds 3072 B of staging per warp: 32 warps of a 2-CTA launch need 96 KB, which still fits twice
     const int warps = pl.threads / 32;
@@ -71,16 +80,29 @@ cudaError_t launch_ramp_fused_ilp(double* z, double* d, size_t n, unsigned int n
     kern<<<tr->sm_count * pl.ctas_per_sm, pl.threads, smem, st>>>(
         z, d, n, nsteps, item_steps, first, last, pl.dynamic, tr->sched,
         reinterpret_cast<unsigned int*>(tr->sched + 1), tr->c64,
-        reinterpret_cast<const double2*>(reinterpret_cast<const RampEntry*>(tr->ramp_table) + (SPLIT ? 0 : 1)));
+        SCALED ? reinterpret_cast<const double2*>(scaled_table(tr)) : reinterpret_cast<const double2*>(tr->ramp_table),
+        flag);
     return cudaGetLastError();
 }
 
+// layout: 0 the plain layout only (split drifts, or no RF at all); 1 the scaled layout only (no
+// voltage table: the kick amplitude cannot vanish); 2 both launches, the device flag picks one
 template <int HARM, bool SPLIT>
 cudaError_t launch_ramp_fused(double* z, double* d, size_t n, unsigned int nsteps, unsigned int item_steps,
                               int first, int last, const PersistentPlan& pl, const lt_tracker* tr,
-                              cudaStream_t st) {
-    if (pl.ilp == 2) return launch_ramp_fused_ilp<HARM, SPLIT, 2>(z, d, n, nsteps, item_steps, first, last, pl, tr, st);
-    return launch_ramp_fused_ilp<HARM, SPLIT, 1>(z, d, n, nsteps, item_steps, first, last, pl, tr, st);
+                              int layout, cudaStream_t st) {
+    const unsigned int* flag = layout == 2 ? layout_flag(tr) : nullptr;
+    cudaError_t e = cudaSuccess;
+    if (SPLIT || layout != 1) {
+        e = pl.ilp == 2 ? launch_ramp_fused_ilp<HARM, SPLIT, 2, false>(z, d, n, nsteps, item_steps, first, last, pl, tr, flag, st)
+                        : launch_ramp_fused_ilp<HARM, SPLIT, 1, false>(z, d, n, nsteps, item_steps, first, last, pl, tr, flag, st);
+        if (e != cudaSuccess) return e;
+    }
+    if (!SPLIT && layout != 0) {
+        e = pl.ilp == 2 ? launch_ramp_fused_ilp<HARM, false, 2, true>(z, d, n, nsteps, item_steps, first, last, pl, tr, flag, st)
+                        : launch_ramp_fused_ilp<HARM, false, 1, true>(z, d, n, nsteps, item_steps, first, last, pl, tr, flag, st);
+    }
+    return e;
 }
 
 template <int HARM, int NSUB>
@@ -152,6 +174,18 @@ int lt_track_ramp(lt_tracker* tr, double* z, double* d, size_t n, unsigned long 
     if (rc) return rc;
     const PersistentPlan pl = plan_persistent(tr, n, turns, 2);
     const RampRing R = make_ring(tr);
+    // which fast layout: the scaled one divides by the kick amplitude tau a_t A(p) of every sub-step
+    int layout = 0;
+    if (!split && R.qV != 0.0 && tr->ramp_scaled != 0) {
+        layout = volt ? 2 : 1;
+        if (layout == 2) {
+            LT_CUDA(tr, cudaMemsetAsync(layout_flag(tr), 0, sizeof(unsigned int), st));
+            const unsigned int blocks = (unsigned int)std::min<unsigned long long>((turns + 255) / 256, 1024);
+            ramp_scan_kernel<<<blocks, 256, 0, st>>>(volt, turns, layout_flag(tr));
+            LT_CUDA(tr, cudaGetLastError());
+            tr->launches++;
+        }
+    }
     unsigned long long done = 0;
     while (done < turns) {
         const unsigned long long chunk = std::min<unsigned long long>(turns - done, chunk_max);
@@ -161,19 +195,19 @@ int lt_track_ramp(lt_tracker* tr, double* z, double* d, size_t n, unsigned long 
         // the table of the previous chunk is free again: its kernel precedes this one on the stream
         ramp_pack_kernel<<<(unsigned)((chunk + 255) / 256), 256, 0, st>>>(
             p0c, volt, phase, done, (unsigned int)chunk, turns, tr->p.integrator, split ? 0 : 1, R,
-            reinterpret_cast<RampEntry*>(tr->ramp_table));
+            reinterpret_cast<RampEntry*>(tr->ramp_table), layout ? scaled_table(tr) : nullptr);
         LT_CUDA(tr, cudaGetLastError());
         if (pl.dynamic) LT_CUDA(tr, cudaMemsetAsync(tr->sched, 0, 8 + 4 * ((n + 31) / 32), st));
         const unsigned int nsteps = (unsigned int)chunk * nsub, item_steps = item_turns * nsub;
         cudaError_t e;
         if (tr->harm == 1)
-            e = split ? launch_ramp_fused<1, true>(z, d, n, nsteps, item_steps, first, last, pl, tr, st)
-                      : launch_ramp_fused<1, false>(z, d, n, nsteps, item_steps, first, last, pl, tr, st);
+            e = split ? launch_ramp_fused<1, true>(z, d, n, nsteps, item_steps, first, last, pl, tr, layout, st)
+                      : launch_ramp_fused<1, false>(z, d, n, nsteps, item_steps, first, last, pl, tr, layout, st);
         else
-            e = split ? launch_ramp_fused<2, true>(z, d, n, nsteps, item_steps, first, last, pl, tr, st)
-                      : launch_ramp_fused<2, false>(z, d, n, nsteps, item_steps, first, last, pl, tr, st);
+            e = split ? launch_ramp_fused<2, true>(z, d, n, nsteps, item_steps, first, last, pl, tr, layout, st)
+                      : launch_ramp_fused<2, false>(z, d, n, nsteps, item_steps, first, last, pl, tr, layout, st);
         LT_CUDA(tr, e);
-        tr->launches += 2;
+        tr->launches += layout == 2 ? 3 : 2;
         done += chunk;
     }
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
@@ -207,7 +241,7 @@ int lt_track_ramp_per_turn(lt_tracker* tr, double* z, double* d, size_t n, unsig
         const unsigned int cnt = (unsigned int)std::min<unsigned long long>(1ULL << 20, turns - off);
         ramp_pack_kernel<<<(cnt + 255) / 256, 256, 0, st>>>(
             p0c, volt, phase, off, cnt, turns, tr->p.integrator, 0, R,
-            reinterpret_cast<RampEntry*>(tr->ramp_table) + (size_t)off * nsub);
+            reinterpret_cast<RampEntry*>(tr->ramp_table) + (size_t)off * nsub, nullptr);
         LT_CUDA(tr, cudaGetLastError());
         tr->launches++;
     }

@@ -96,6 +96,42 @@ def test_ramp_split_drift_fused_equals_per_turn_bits_and_chunking_is_invisible(i
 
 
 @pytest.mark.parametrize("integrator", INTEGRATORS)
+def test_ramp_scaled_and_plain_fast_layouts(integrator):
+    """Merged-drift fused mode has two layouts: delta divided by the running kick amplitude (15 FP64
+    instructions per sub-step, the default) and the plain one (16).  Both must sit inside the 1e-9
+    gate against the oracle, with and without a voltage table; a voltage table that contains a
+    ZERO cannot be divided by: the device-side scan of the table then selects the plain layout
+    for the whole call, whose bits the result must equal -- also when the call is chunked and
+    the zero sits in a later chunk than the first."""
+    N = 700
+    p0c, a, psi = wl.energy_ramp(N, 26e9, 26.2e9)
+    a = a * (1.0 + 0.3 * np.sin(np.arange(N) / 40.0))
+    for r in (0.0, 0.5):
+        tr, p = both(integrator, r)
+        z0, d0 = wl.gaussian_bunch(4001, 0.1, 71, ratio2=r)
+        for volt in (a, None):
+            zo, do = oracle.track_ramp(p, z0, d0, p0c, volt, psi)
+            out = {}
+            for scaled in (0, 1):
+                tr.set_option(lt.OPT_RAMP_SCALED, scaled)
+                out[scaled] = gpu_ramp(tr, z0, d0, p0c, volt, psi)
+                assert_close(p, out[scaled][0], out[scaled][1], zo, do)
+            assert not np.array_equal(out[0][1], out[1][1])          # they really are two evaluation orders
+        a0 = a.copy()
+        a0[[450, 451, 699]] = 0.0                                    # the RF is off for three turns
+        zo, do = oracle.track_ramp(p, z0, d0, p0c, a0, psi)
+        tr.set_option(lt.OPT_RAMP_SCALED, 0)
+        ref = gpu_ramp(tr, z0, d0, p0c, a0, psi)
+        assert_close(p, ref[0], ref[1], zo, do)
+        tr.set_option(lt.OPT_RAMP_SCALED, 1)
+        for chunk in (1 << 22, 128):
+            tr.set_option(lt.OPT_CHUNK_TURNS, chunk)
+            got = gpu_ramp(tr, z0, d0, p0c, a0, psi)
+            assert np.array_equal(got[0], ref[0]) and np.array_equal(got[1], ref[1]), chunk
+        tr.set_option(lt.OPT_CHUNK_TURNS, 1 << 22)
+
+
+@pytest.mark.parametrize("integrator", INTEGRATORS)
 def test_flat_ramp_without_tables_is_the_plain_map(integrator):
     """p0c constant at the create value, NULL tables: the plain map up to the rounding of
     beta(p) vs beta(gamma) (not bits: A and d are recomputed from p)."""
