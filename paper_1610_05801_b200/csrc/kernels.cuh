@@ -20,7 +20,7 @@
 namespace lt {
 
 #ifndef LT_TURN_UNROLL
-#define LT_TURN_UNROLL 16
+#define LT_TURN_UNROLL 96     // particle-turns per iteration of the fused single-harmonic turn loop (see advance())
 #endif
 
 constexpr int kEulerCromer = 0, kLeapfrog = 1, kRuth4 = 2;
@@ -351,7 +351,12 @@ __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int 
             }
         }
         // every non-FP64 instruction costs issue capacity next to the saturated FP64 pipe
-        // (profiles/r2_fp64_pipe_probe.md): unroll deep enough that the loop counter disappears
+        // (profiles/r2_fp64_pipe_probe.md): the loop's 8 instructions of overhead (5 uniform-register
+        // reloads, counter, compare, branch) are spread over LT_TURN_UNROLL particle-turns.  Configs[1]:
+        // 16 particle-turns per iteration 0.905 of the FP64 peak, 64: 0.912, 128: 0.915 -- and 256
+        // (57 KB of code): 0.59, the loop no longer fits the instruction cache; the default keeps a
+        // third of headroom below the largest body that measured well.  The double harmonic and
+        // Ruth4 measured BEST at 4 turns per iteration (longer bodies cost them 1.5-2 points).
         constexpr int kUnroll = (INTEG == kRuth4 || HARM != 1 || ILP > 2) ? 4 : LT_TURN_UNROLL / ILP;
 #pragma unroll kUnroll
         for (unsigned int t = 1; t < turns; ++t) {
