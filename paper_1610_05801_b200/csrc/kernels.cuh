@@ -356,8 +356,16 @@ __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int 
         // 16 particle-turns per iteration 0.905 of the FP64 peak, 64: 0.912, 128: 0.915 -- and 256
         // (57 KB of code): 0.59, the loop no longer fits the instruction cache; the default keeps a
         // third of headroom below the largest body that measured well.  The double harmonic and
-        // Ruth4 measured BEST at 4 turns per iteration (longer bodies cost them 1.5-2 points).
-        constexpr int kUnroll = (INTEG == kRuth4 || HARM != 1 || ILP > 2) ? 4 : LT_TURN_UNROLL / ILP;
+        // Ruth4 measured BEST at 4 turns per iteration in fp64 (2: -2 points, 8: -1.5) and at 2 in the
+        // packed fp32 kernels (0.864 of the FP32 peak against 0.845 at 4, 0.83 at 1 and 3).
+#ifndef LT_UNROLL_OTHER
+#define LT_UNROLL_OTHER 4
+#endif
+#ifndef LT_UNROLL_OTHER_F32
+#define LT_UNROLL_OTHER_F32 2
+#endif
+        constexpr int kOther = sizeof(T) == 8 && R::NS == 8 ? LT_UNROLL_OTHER : LT_UNROLL_OTHER_F32;   // fp64 : fp32 (scalar or packed)
+        constexpr int kUnroll = (INTEG == kRuth4 || HARM != 1 || ILP > 2) ? kOther : LT_TURN_UNROLL / ILP;
 #pragma unroll kUnroll
         for (unsigned int t = 1; t < turns; ++t) {
 #pragma unroll
