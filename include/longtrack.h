@@ -162,7 +162,8 @@ enum {
                                   0 on the argument, 1 on the polynomial; same bits either way */
     LT_OPT_RAMP_SCALED    = 12 /* lt_track_ramp, merged drifts: 1 (default) carries delta divided by
                                   the running kick amplitude (15 FP64 instructions per sub-step,
-                                  four table values) whenever no voltage scale of the call is zero;
+                                  four table values) unless a voltage scale of the call is zero, not
+                                  finite or beyond 1e+-100 (scanned on the device, per call);
                                   0 always the plain form (16 instructions, five values).  The two
                                   round differently (both far inside the 1e-9 gate).              */
 };

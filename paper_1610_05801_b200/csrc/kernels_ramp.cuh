@@ -89,13 +89,14 @@ __device__ __forceinline__ double ramp_ga(const RampTurn& t, int k, double av) {
     return ramp_g(t, k) * (t.tau[k] * t.A[k] * av);
 }
 
-// *flag |= 1 when any voltage scale of the call is zero (the scaled layout divides by the kick amplitude)
+// *flag |= 1 when any voltage scale of the call is zero, not finite or beyond 1e+-100 (the scaled
+// layout divides by the kick amplitude)
 static __global__ void ramp_scan_kernel(const double* __restrict__ volt, unsigned long long turns,
                                         unsigned int* __restrict__ flag) {
     bool zero = false;
     for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < turns;
          i += (unsigned long long)gridDim.x * blockDim.x)
-        zero |= !(fabs(volt[i]) > 0.0);                        // zero or NaN
+        zero |= !(fabs(volt[i]) > 1e-100 && fabs(volt[i]) < 1e100);   // zero, NaN, or so extreme that delta / amp could leave the fp64 range
     if (__syncthreads_or(zero) && threadIdx.x == 0) atomicOr(flag, 1u);
 }
 
