@@ -160,12 +160,17 @@ enum {
                                   per lane at most 4)                                               */
     LT_OPT_FLIP_ON_Q      = 11,/* where the sign of the reduced sine is applied: -1 planner,
                                   0 on the argument, 1 on the polynomial; same bits either way */
-    LT_OPT_RAMP_SCALED    = 12 /* lt_track_ramp, merged drifts: 1 (default) carries delta divided by
+    LT_OPT_RAMP_SCALED    = 12,/* lt_track_ramp, merged drifts: 1 (default) carries delta divided by
                                   the running kick amplitude (15 FP64 instructions per sub-step,
                                   four table values) unless a voltage scale of the call is zero, not
                                   finite or beyond 1e+-100 (scanned on the device, per call);
                                   0 always the plain form (16 instructions, five values).  The two
                                   round differently (both far inside the 1e-9 gate).              */
+    LT_OPT_LATTICE_SOURCE = 13 /* where the fused transverse kernel keeps the lattice: 0 (default)
+                                  planner -- the kernel-parameter space (constant bank, uniform
+                                  registers) for lattices of at most 24 segments, else shared
+                                  memory; 1 shared memory; 2 parameter space (longer lattices
+                                  still use shared memory).  Same bits either way.              */
 };
 
 /* Counters for lt_get_stat. */

@@ -570,6 +570,7 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
             __syncwarp();
             if (lane == 0) st_release_u32(done + g, publish);
         }
+        __syncwarp();            // the warp is converged again before the next piece (see run_piece's callers)
     };
 
     if (dynamic == 2) {
@@ -591,7 +592,8 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
             const unsigned long long gx = g * (unsigned long long)turns;
             const unsigned int t_end = (unsigned int)(x - gx);
             const unsigned int t_begin = x_lo > gx ? (unsigned int)(x_lo - gx) : 0u;
-            run_piece(g, t_begin, t_end - t_begin, t_begin ? 1u : 0u, t_end < turns ? 1u : 0u);
+            run_piece(__shfl_sync(0xffffffffu, g, 0), __shfl_sync(0xffffffffu, t_begin, 0),
+                      __shfl_sync(0xffffffffu, t_end - t_begin, 0), t_begin ? 1u : 0u, t_end < turns ? 1u : 0u);
             x = gx + t_begin;
         }
         return;
@@ -607,10 +609,12 @@ fused_persistent_kernel(T* __restrict__ z_arr, T* __restrict__ d_arr, size_t n, 
         unsigned long long t = next;
         if (dynamic) {
             if (lane == 0) t = atomicAdd(ticket, 1ULL);
-            t = __shfl_sync(0xffffffffu, t, 0);
         } else {
             next += slots;
         }
+        // in static mode too: the broadcast tells ptxas that the work item, and every loop below
+        // it, is warp-uniform (counters and table addresses then live in uniform registers)
+        t = __shfl_sync(0xffffffffu, t, 0);
         if (t >= total) break;
         const unsigned int c = (unsigned int)(t / groups);
         const unsigned long long g = t - (unsigned long long)c * groups;

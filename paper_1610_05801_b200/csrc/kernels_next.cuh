@@ -350,27 +350,72 @@ __device__ __forceinline__ void transverse_turn(double (&u)[ILP][4], unsigned in
     }
 }
 
+// The lattice as a KERNEL PARAMETER (constant bank), for lattices of up to kParamSegments segments:
+// inside a segment loop that is NOT unrolled, ptxas fetches the 16 elements of the segment with
+// uniform loads (LDCU c[0x0][UR + off]) into uniform registers and every FP64 instruction of the
+// matrix product takes the form  DFMA R, R, UR, R  -- two vector-register operands, which the FP64
+// pipe issues every 2.00 cycles, against 2.17 for the three-register form a matrix element fetched
+// from shared memory forces (profiles/r2_fp64_pipe_probe.md) -- and no shared-memory loads at all.
+// Two conditions, both found by bisecting the SASS: (1) the segment count is read from the
+// parameter struct itself and the loop is not unrolled (unrolled, ptxas hoists the loads out of
+// the turn loop into vector registers and moves them back with R2UR, spilling); (2) ptxas must
+// see the work item as warp-uniform and the warp CONVERGED around the turn loop: the item index is
+// broadcast with __shfl_sync in every scheduling mode, and the work-item loop ends in a
+// __syncwarp() -- a trailing `if (lane == 0) store` without one is enough to make ptxas keep the
+// segment counter in a vector register and fetch the elements with LDC into vector registers
+// (0.74 of the peak instead of 0.88).
+constexpr int kParamSegments = 24;                      // 3 KB of the 4 KB parameter space
+struct LatticeParam { double m[kParamSegments][16]; int n_seg; };
+
+template <int ILP>
+__device__ __forceinline__ void apply_matrix_param(double (&u)[ILP][4], const double (&M)[16]) {
+    double w[ILP][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) {
+            double acc = __dmul_rn(M[4 * i], u[j][0]);
+            acc = __fma_rn(M[4 * i + 1], u[j][1], acc);
+            acc = __fma_rn(M[4 * i + 2], u[j][2], acc);
+            w[j][i] = __fma_rn(M[4 * i + 3], u[j][3], acc);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < ILP; ++j)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) u[j][i] = w[j][i];
+}
+
+// where a kernel's lattice lives: shared memory (any length) or the parameter space
+struct LatticeInShared {
+    unsigned int base; int n_seg;
+    template <int NSEG, int ILP> __device__ __forceinline__ void turn(double (&u)[ILP][4]) const {
+        transverse_turn<NSEG, ILP>(u, base, n_seg);
+    }
+};
+struct LatticeInParam {
+    const LatticeParam& L;
+    template <int NSEG, int ILP> __device__ __forceinline__ void turn(double (&u)[ILP][4]) const {
+#pragma unroll 1
+        for (int s = 0; s < L.n_seg; ++s) apply_matrix_param<ILP>(u, L.m[s]);
+    }
+};
+
 // Fused multi-turn transverse kernel: the persistent, ticketed work queue of
 // fused_persistent_kernel (items = chunk of item_turns turns x group of 32*ILP particles) with the
 // four transverse coordinates -- and, when LONGI, the leap-frog single-harmonic longitudinal
 // turn of the same particle (fast path: phase state, merged drifts) -- held in registers.
 // Particle j of a lane is element  g*32*ILP + j*32 + lane  (coalesced).  The arithmetic per
 // particle does not depend on ILP, so every launch shape returns the same bits.
-template <int NSEG, bool LONGI, int ILP>
-__global__ void __launch_bounds__(ILP == 1 ? 1024 : (ILP == 8 ? 256 : 512), 1)
-transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp_arr,
+template <int NSEG, bool LONGI, int ILP, typename LAT>
+__device__ __forceinline__ void
+transverse_persistent_body(double* __restrict__ x_arr, double* __restrict__ xp_arr,
                              double* __restrict__ y_arr, double* __restrict__ yp_arr,
                              double* __restrict__ z_arr, double* __restrict__ d_arr, size_t n,
                              unsigned int turns, unsigned int item_turns, int first_launch,
                              int last_launch, int dynamic, unsigned long long* __restrict__ ticket,
-                             unsigned int* __restrict__ done, const double* __restrict__ Mg,
-                             int n_seg, const __grid_constant__ MapConsts<double> P) {
-    // dynamic shared memory: the lattice; the request is padded to cap the CTAs per SM
-    extern __shared__ double2 lattice2[];
-    for (int k = threadIdx.x; k < 8 * n_seg; k += blockDim.x)
-        lattice2[k] = __ldg(reinterpret_cast<const double2*>(Mg) + k);
-    __syncthreads();
-    const unsigned int lat = (unsigned int)__cvta_generic_to_shared(lattice2);
+                             unsigned int* __restrict__ done, const LAT lat,
+                             const MapConsts<double>& P) {
     constexpr unsigned int G = 32u * ILP;
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned long long groups = (n + G - 1) / G;
@@ -384,10 +429,12 @@ transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp
         unsigned long long t = next;
         if (dynamic) {
             if (lane == 0) t = atomicAdd(ticket, 1ULL);
-            t = __shfl_sync(0xffffffffu, t, 0);
         } else {
             next += slots;
         }
+        // also in static mode, where every lane already holds the same t: the broadcast is what
+        // tells ptxas that the work item -- and with it every loop below -- is warp-uniform
+        t = __shfl_sync(0xffffffffu, t, 0);
         if (t >= total) break;
         const unsigned int c = (unsigned int)(t / groups);
         const unsigned long long g = t - (unsigned long long)c * groups;
@@ -417,14 +464,14 @@ transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp
         }
 #pragma unroll 1
         for (unsigned int k = 1; k < nt; ++k) {
-            transverse_turn<NSEG, ILP>(u, lat, n_seg);
+            lat.template turn<NSEG, ILP>(u);
             if (LONGI) {
 #pragma unroll
                 for (int j = 0; j < ILP; ++j)
                     turn_fast<double, kLeapfrog, 1, true>(v[j], dl[j], P, P.drift_merged);
             }
         }
-        transverse_turn<NSEG, ILP>(u, lat, n_seg);
+        lat.template turn<NSEG, ILP>(u);
 #pragma unroll
         for (int j = 0; j < ILP; ++j) {
             const size_t i = i0 + 32u * j;
@@ -443,7 +490,44 @@ transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp
             __syncwarp();
             if (lane == 0) st_release_u32(done + g, c + 1);
         }
+        __syncwarp();            // ptxas must see the warp converged at the next work item (LatticeInParam)
     }
+}
+
+template <int NSEG, bool LONGI, int ILP>
+__global__ void __launch_bounds__(ILP == 1 ? 1024 : (ILP == 8 ? 256 : 512), 1)
+transverse_persistent_kernel(double* __restrict__ x_arr, double* __restrict__ xp_arr,
+                             double* __restrict__ y_arr, double* __restrict__ yp_arr,
+                             double* __restrict__ z_arr, double* __restrict__ d_arr, size_t n,
+                             unsigned int turns, unsigned int item_turns, int first_launch,
+                             int last_launch, int dynamic, unsigned long long* __restrict__ ticket,
+                             unsigned int* __restrict__ done, const double* __restrict__ Mg,
+                             int n_seg, const __grid_constant__ MapConsts<double> P) {
+    // dynamic shared memory: the lattice; the request is padded to cap the CTAs per SM
+    extern __shared__ double2 lattice2[];
+    for (int k = threadIdx.x; k < 8 * n_seg; k += blockDim.x)
+        lattice2[k] = __ldg(reinterpret_cast<const double2*>(Mg) + k);
+    __syncthreads();
+    const LatticeInShared lat = {(unsigned int)__cvta_generic_to_shared(lattice2), n_seg};
+    transverse_persistent_body<NSEG, LONGI, ILP>(x_arr, xp_arr, y_arr, yp_arr, z_arr, d_arr, n, turns, item_turns,
+                                                 first_launch, last_launch, dynamic, ticket, done, lat, P);
+}
+
+// the same kernel with the lattice in the parameter space (n_seg <= kParamSegments)
+template <bool LONGI, int ILP>
+__global__ void __launch_bounds__(ILP == 1 ? 1024 : (ILP == 8 ? 256 : 512), 1)
+transverse_persistent_param_kernel(double* __restrict__ x_arr, double* __restrict__ xp_arr,
+                                   double* __restrict__ y_arr, double* __restrict__ yp_arr,
+                                   double* __restrict__ z_arr, double* __restrict__ d_arr, size_t n,
+                                   unsigned int turns, unsigned int item_turns, int first_launch,
+                                   int last_launch, int dynamic, unsigned long long* __restrict__ ticket,
+                                   unsigned int* __restrict__ done,
+                                   const __grid_constant__ LatticeParam Lp,
+                                   const __grid_constant__ MapConsts<double> P) {
+    extern __shared__ double2 lattice2[];               // residency cap only
+    const LatticeInParam lat = {Lp};
+    transverse_persistent_body<0, LONGI, ILP>(x_arr, xp_arr, y_arr, yp_arr, z_arr, d_arr, n, turns, item_turns,
+                                              first_launch, last_launch, dynamic, ticket, done, lat, P);
 }
 
 // Per-turn transverse kernel: ONE turn per launch, all coordinates through HBM -- 64 B per

@@ -371,6 +371,7 @@ ramp_persistent_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, s
             __syncwarp();
             if (lane == 0) st_release_u32(done + g, publish);
         }
+        __syncwarp();            // the warp is converged again before the next piece (see run_piece's callers)
     };
 
     if (dynamic == 2) {                       // wrap-around schedule, see fused_persistent_kernel
@@ -382,7 +383,8 @@ ramp_persistent_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, s
             const unsigned long long gx = g * (unsigned long long)nsteps;
             const unsigned int s_end = (unsigned int)(x - gx);
             const unsigned int s_begin = x_lo > gx ? (unsigned int)(x_lo - gx) : 0u;
-            run_piece(g, s_begin, s_end - s_begin, s_begin ? 1u : 0u, s_end < nsteps ? 1u : 0u);
+            run_piece(__shfl_sync(0xffffffffu, g, 0), __shfl_sync(0xffffffffu, s_begin, 0),
+                      __shfl_sync(0xffffffffu, s_end - s_begin, 0), s_begin ? 1u : 0u, s_end < nsteps ? 1u : 0u);
             x = gx + s_begin;
         }
         return;
@@ -397,10 +399,12 @@ ramp_persistent_kernel(double* __restrict__ z_arr, double* __restrict__ d_arr, s
         unsigned long long t = next;
         if (dynamic) {
             if (lane == 0) t = atomicAdd(ticket, 1ULL);
-            t = __shfl_sync(0xffffffffu, t, 0);
         } else {
             next += slots;
         }
+        // in static mode too: the broadcast tells ptxas that the work item, and every loop below
+        // it, is warp-uniform (counters and table addresses then live in uniform registers)
+        t = __shfl_sync(0xffffffffu, t, 0);
         if (t >= total) break;
         const unsigned int c = (unsigned int)(t / groups);
         const unsigned long long g = t - (unsigned long long)c * groups;

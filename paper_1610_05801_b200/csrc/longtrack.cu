@@ -745,6 +745,9 @@ int lt_set_option(lt_tracker* tr, int option, long long value) {
             if (value < -1 || value > 1) return LT_E_PARAM;
             tr->flip_on_q = value; return LT_OK;
         case LT_OPT_RAMP_SCALED: tr->ramp_scaled = value != 0; return LT_OK;
+        case LT_OPT_LATTICE_SOURCE:
+            if (value < 0 || value > 2) return LT_E_PARAM;
+            tr->lattice_source = value; return LT_OK;
         default: return LT_E_PARAM;
     }
 }
@@ -764,6 +767,7 @@ int lt_get_option(const lt_tracker* tr, int option, long long* value) {
         case LT_OPT_WARPS_PER_SMSP: *value = tr->warps_per_smsp; return LT_OK;
         case LT_OPT_FLIP_ON_Q: *value = tr->flip_on_q; return LT_OK;
         case LT_OPT_RAMP_SCALED: *value = tr->ramp_scaled; return LT_OK;
+        case LT_OPT_LATTICE_SOURCE: *value = tr->lattice_source; return LT_OK;
         default: return LT_E_PARAM;
     }
 }

@@ -369,10 +369,34 @@ cudaError_t launch_transverse_one(double* x, double* xp, double* y, double* yp, 
     return cudaGetLastError();
 }
 
+// lattice in the parameter space (constant bank -> uniform registers; kernels_next.cuh)
+template <bool LONGI, int ILP>
+cudaError_t launch_transverse_param(double* x, double* xp, double* y, double* yp, double* z, double* d,
+                                    size_t n, unsigned int turns, unsigned int item_turns, int first, int last,
+                                    const PersistentPlan& pl, const lt_tracker* tr, cudaStream_t st) {
+    auto kern = transverse_persistent_param_kernel<LONGI, ILP>;
+    const int smem = residency_smem(pl);
+    static bool attr_set = false;                        // once per instantiation
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    LatticeParam lp;
+    std::memcpy(lp.m, tr->lattice_host, (size_t)tr->n_seg * 16 * sizeof(double));
+    lp.n_seg = tr->n_seg;
+    kern<<<tr->sm_count * pl.ctas_per_sm, pl.threads, smem, st>>>(
+        x, xp, y, yp, z, d, n, turns, item_turns, first, last, pl.dynamic, tr->sched,
+        reinterpret_cast<unsigned int*>(tr->sched + 1), lp, tr->c64);
+    return cudaGetLastError();
+}
+
 template <bool LONGI, int ILP>
 cudaError_t launch_transverse_ilp(double* x, double* xp, double* y, double* yp, double* z, double* d,
                                   size_t n, unsigned int turns, unsigned int item_turns, int first, int last,
                                   const PersistentPlan& pl, const lt_tracker* tr, cudaStream_t st) {
+    if (tr->lattice_source != 1 && tr->n_seg <= kParamSegments)
+        return launch_transverse_param<LONGI, ILP>(x, xp, y, yp, z, d, n, turns, item_turns, first, last, pl, tr, st);
 #define LT_TV(NS) launch_transverse_one<NS, LONGI, ILP>(x, xp, y, yp, z, d, n, turns, item_turns, first, last, pl, tr, st)
     switch (tr->n_seg <= kSegUnrolled ? tr->n_seg : 0) {
         case 1: return LT_TV(1);

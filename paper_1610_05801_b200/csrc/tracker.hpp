@@ -56,7 +56,7 @@ struct lt_tracker {
     int harm;                 // 0 generic (phi_s != 0), 1 single, 2 double harmonic
     // options
     long long split_drifts, chunk_turns, fused_ilp, fused_block, per_turn_graph,
-        per_turn_ctas_per_sm, per_turn_reverse, fused_mode, item_turns, warps_per_smsp, flip_on_q, ramp_scaled;
+        per_turn_ctas_per_sm, per_turn_reverse, fused_mode, item_turns, warps_per_smsp, flip_on_q, ramp_scaled, lattice_source;
     // stats
     long long launches, last_grid, last_block, last_ilp, last_mode, last_item_turns;
     int sm_count;             // 0 until the first device call

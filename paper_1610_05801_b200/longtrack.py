@@ -29,6 +29,7 @@ OPT_SPLIT_DRIFTS, OPT_CHUNK_TURNS, OPT_FUSED_ILP, OPT_FUSED_BLOCK = 1, 2, 3, 4
 OPT_PER_TURN_GRAPH, OPT_PER_TURN_CTAS_PER_SM, OPT_PER_TURN_REVERSE = 5, 6, 7
 OPT_FUSED_MODE, OPT_ITEM_TURNS, OPT_WARPS_PER_SMSP, OPT_FLIP_ON_Q = 8, 9, 10, 11
 OPT_RAMP_SCALED = 12
+OPT_LATTICE_SOURCE = 13
 FUSED_AUTO, FUSED_PLAIN, FUSED_PERSISTENT_STATIC, FUSED_PERSISTENT_DYNAMIC = 0, 1, 2, 3
 FUSED_PERSISTENT_WRAP = 4
 STAT_KERNEL_LAUNCHES, STAT_LAST_GRID, STAT_LAST_BLOCK, STAT_LAST_ILP, STAT_SM_COUNT = 1, 2, 3, 4, 5

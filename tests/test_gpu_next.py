@@ -519,12 +519,13 @@ def test_transverse_chunking_is_invisible_and_misaligned_arrays_work():
         tr.track_transverse_fused(arrays[0], arrays[1], arrays[2], arrays[3], None, None, n, 1, stream_ptr())
 
 
-@pytest.mark.parametrize("n_seg", [4, 6])
+@pytest.mark.parametrize("n_seg", [4, 6, 24, 25])
 def test_transverse_every_ilp_shape_returns_the_same_bits(n_seg):
     """1, 2, 4 or 8 particles per lane (8: 256 threads and 220 registers per thread, the planner's
     choice from 3*10^5 particles on), static slots or the ticket queue, unrolled (<= 4 segments) or
-    looped lattice: the arithmetic per particle is the same, so the six arrays must be
-    bit-identical, on a ragged n that leaves the last group partly empty."""
+    looped lattice, lattice in shared memory or in the kernel-parameter space (at most 24 segments;
+    25 silently stays in shared memory): the arithmetic per particle is the same, so the six arrays
+    must be bit-identical, on a ragged n that leaves the last group partly empty."""
     tr, p = both()
     mats, twiss = wl.transverse_lattice(n_seg, 60 + n_seg)
     n = 40_000 + 77
@@ -532,16 +533,18 @@ def test_transverse_every_ilp_shape_returns_the_same_bits(n_seg):
     z0, d0 = wl.gaussian_bunch(n, 0.23, 62)
     tr.set_transverse(mats)
     ref = None
-    for ilp in (1, 2, 4, 8):
-        for mode in (lt.FUSED_PERSISTENT_STATIC, lt.FUSED_PERSISTENT_DYNAMIC):
-            tr.set_option(lt.OPT_FUSED_ILP, ilp)
-            tr.set_option(lt.OPT_FUSED_MODE, mode)
-            tr.set_option(lt.OPT_ITEM_TURNS, 37 if mode == lt.FUSED_PERSISTENT_DYNAMIC else 0)
-            out = gpu_transverse(tr, coords, z0, d0, 211, "fused")
-            assert tr.get_stat(lt.STAT_LAST_ILP) == ilp
-            if ref is None:
-                ref = out
-            assert all(np.array_equal(out[k], ref[k]) for k in range(6)), (ilp, mode)
+    for source in (1, 2):              # lattice in shared memory / in the kernel-parameter space (uniform registers)
+        tr.set_option(lt.OPT_LATTICE_SOURCE, source)
+        for ilp in (1, 2, 4, 8):
+            for mode in (lt.FUSED_PERSISTENT_STATIC, lt.FUSED_PERSISTENT_DYNAMIC):
+                tr.set_option(lt.OPT_FUSED_ILP, ilp)
+                tr.set_option(lt.OPT_FUSED_MODE, mode)
+                tr.set_option(lt.OPT_ITEM_TURNS, 37 if mode == lt.FUSED_PERSISTENT_DYNAMIC else 0)
+                out = gpu_transverse(tr, coords, z0, d0, 211, "fused")
+                assert tr.get_stat(lt.STAT_LAST_ILP) == ilp
+                if ref is None:
+                    ref = out
+                assert all(np.array_equal(out[k], ref[k]) for k in range(6)), (source, ilp, mode)
     idx = np.arange(0, n, 7)
     o = oracle.track_transverse(p, mats, *(c[idx] for c in coords), z0[idx], d0[idx], 211)
     assert_transverse_gate(tuple(r[idx] for r in ref[:4]), o, tuple(c[idx] for c in coords))
