@@ -289,10 +289,11 @@ static __global__ void programme_pack_kernel(const double* __restrict__ volt_sca
 // f3: transverse plane.  One turn = for every segment s in order  u <- M_s u,  u = (x, x', y, y'),
 // M_s row-major; row i is  fma(M_i3, y', fma(M_i2, y, fma(M_i1, x', M_i0 * x)))  -- the
 // association order of the definition, 16 FP64 instructions per segment and particle.
-// sm_100a has no constant-bank operands for DFMA: every matrix element has to sit in a (uniform)
-// register, and 4 matrices are 128 of them.  So the lattice is staged in shared memory and a
-// thread carries ILP particles: each element fetched (or kept in a uniform register by ptxas,
-// which hoists the loads of short lattices out of the turn loop) feeds ILP FMAs.
+// sm_100a has no constant-bank operands for DFMA: every matrix element has to sit in a register.
+// Two homes for the lattice: shared memory (any length; a thread carries ILP particles, so each
+// 16-byte fetch of a matrix row feeds 2*ILP FP64 instructions, all in the three-register form), or
+// the kernel-parameter space for short lattices (LatticeParam below: uniform registers, the
+// two-register form, no fetches from shared memory at all).
 // ------------------------------------------------------------------------------------------
 constexpr int kSegUnrolled = 4;      // lattices up to this length are unrolled at compile time
 
