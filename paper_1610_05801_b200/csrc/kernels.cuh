@@ -75,6 +75,15 @@ template <> struct Real<double> {
         return __hiloint2double((int)hi, __double2loint(f));
     }
     static __device__ __forceinline__ double flip_by(double x, double t) { return flip(x, t); }
+    // (-1)^n as a value, n the integer in the low mantissa bits of t: +-1.0 (one IMAD; the low word is zero)
+    static __device__ __forceinline__ double sign_of(double t) {
+        return __hiloint2double((int)(0x3FF00000u + ((unsigned int)__double2loint(t) << 31)), 0);
+    }
+    // the same, written into the register pair of a previous sign value (whose low word is zero):
+    // one instruction, where sign_of() also has to clear a low word
+    static __device__ __forceinline__ double resign(double prev, double t) {
+        return __hiloint2double((int)(0x3FF00000u + ((unsigned int)__double2loint(t) << 31)), __double2loint(prev));
+    }
 };
 
 template <> struct Real<float> {
@@ -89,6 +98,10 @@ template <> struct Real<float> {
         return __uint_as_float(__float_as_uint(f) + (__float_as_uint(t) << 31));
     }
     static __device__ __forceinline__ float flip_by(float x, float t) { return flip(x, t); }
+    static __device__ __forceinline__ float sign_of(float t) {
+        return __uint_as_float(0x3F800000u + (__float_as_uint(t) << 31));
+    }
+    static __device__ __forceinline__ float resign(float, float t) { return sign_of(t); }
 };
 
 // Two fp32 particles in one 64-bit register pair.  sm_100a has packed FP32 instructions (FFMA2,
@@ -123,6 +136,8 @@ template <> struct Real<f32x2> {
         return f32x2(flip1(f.v.x, t.v.x), flip1(f.v.y, t.v.y));
     }
     static __device__ __forceinline__ f32x2 flip_by(f32x2 x, f32x2 t) { return flip(x, t); }
+    static __device__ __forceinline__ f32x2 sign_of(f32x2 t) { return flip(f32x2(1.0f), t); }
+    static __device__ __forceinline__ f32x2 resign(f32x2, f32x2 t) { return sign_of(t); }
 };
 
 // how many array elements of type T a register value V carries, and access to them
@@ -176,7 +191,7 @@ __device__ __forceinline__ T horner(const T (&c)[N], T s) {
 // with q*a behind the polynomial (same 15 instructions; a = 1 still returns the plain map's bits).
 template <typename T, int HARM, bool FQ = false, int PROG = 0>
 __device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage, T a = T(1),
-                                  T p = T(0)) {
+                                  T p = T(0), T* sg = nullptr) {
     typedef Real<T> R;
     constexpr int NS = R::NS, NC = R::NC;
     static_assert(PROG >= 0 && PROG <= 2, "the energy ramp has its own kick (kernels_ramp.cuh)");
@@ -197,10 +212,14 @@ __device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage
         T fa = PROG ? R::mul(f, a) : f;
         T q = horner<T, NS>(sin_coef, s);         // tau A sin(pi f)/f
         T c = horner<T, NC>(P.cos1, s);           // cos(pi f)
-        // sin and cos both change sign with the parity of n: flip f, and flip 2r for the cos
-        T m = R::fma(R::flip_by(P.two_r, t), c, T(1));
-        if (FQ) return R::fma(fa, R::flip(R::mul(q, m), t), delta);
-        return R::fma(R::flip(fa, t), R::mul(q, m), delta);
+        // sin and cos both change sign with the parity of n:  sigma s (1 + 2 r sigma c) = s (sigma + 2 r c),
+        // so ONE sign value sigma = +-1 does for both (it was a flip of f and a flip of 2r; the bits are
+        // the same: a sign moved through a product or an FMA commutes with the rounding)
+        // sg (fused turn loop): the particle's previous sign value, overwritten in place
+        const T sigma = sg ? R::resign(*sg, t) : R::sign_of(t);
+        if (sg) *sg = sigma;
+        T m = R::fma(P.two_r, c, sigma);
+        return R::fma(fa, R::mul(q, m), delta);
     } else {
         T t1, t2;
         T f1 = reduce_half_periods(R::add(v, P.phi_off), &t1);
@@ -252,20 +271,20 @@ __device__ __forceinline__ void turn_exact(T& z, T& delta, const MapConsts<T>& P
 // offset costs one FP64 instruction and none on the dependent chain.
 template <typename T, int INTEG, int HARM, bool FQ = false, bool PROG = false>
 __device__ __forceinline__ void turn_fast(T& v, T& delta, const MapConsts<T>& P, T trailing,
-                                          T a = T(1), T dp = T(0)) {
+                                          T a = T(1), T dp = T(0), T* sg = nullptr) {
     typedef Real<T> R;
     constexpr int PK = PROG ? 2 : 0;
     if (INTEG == kRuth4) {
-        delta = kick<T, HARM, FQ, PK>(v, delta, P, 0, a);
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 0, a, T(0), sg);
         v = R::fma(-P.drift_mid, delta, v);
-        delta = kick<T, HARM, FQ, PK>(v, delta, P, 1, a);
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 1, a, T(0), sg);
         v = R::fma(-P.drift_mid, delta, v);
         const T w = PROG ? R::add(v, dp) : v;
-        delta = kick<T, HARM, FQ, PK>(v, delta, P, 2, a);
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 2, a, T(0), sg);
         v = R::fma(-trailing, delta, w);
     } else {
         const T w = PROG ? R::add(v, dp) : v;
-        delta = kick<T, HARM, FQ, PK>(v, delta, P, 0, a);
+        delta = kick<T, HARM, FQ, PK>(v, delta, P, 0, a, T(0), sg);
         v = R::fma(-trailing, delta, w);
     }
 }
@@ -366,16 +385,19 @@ __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int 
 #endif
         constexpr int kOther = sizeof(T) == 8 && R::NS == 8 ? LT_UNROLL_OTHER : LT_UNROLL_OTHER_F32;   // fp64 : fp32 (scalar or packed)
         constexpr int kUnroll = (INTEG == kRuth4 || HARM != 1 || ILP > 2) ? kOther : LT_TURN_UNROLL / ILP;
+        T sg[ILP];                           // double harmonic: the particles' sign values (see kick)
+#pragma unroll
+        for (int j = 0; j < ILP; ++j) sg[j] = T(1);
 #pragma unroll kUnroll
         for (unsigned int t = 1; t < turns; ++t) {
 #pragma unroll
             for (int j = 0; j < ILP; ++j)
-                turn_fast<T, INTEG, HARM, FQ, false>(x[j], dl[j], P, P.drift_merged);
+                turn_fast<T, INTEG, HARM, FQ, false>(x[j], dl[j], P, P.drift_merged, T(1), T(0), &sg[j]);
         }
         const T trailing = last ? P.drift_trail : P.drift_merged;
 #pragma unroll
         for (int j = 0; j < ILP; ++j) {
-            turn_fast<T, INTEG, HARM, FQ, false>(x[j], dl[j], P, trailing);
+            turn_fast<T, INTEG, HARM, FQ, false>(x[j], dl[j], P, trailing, T(1), T(0), &sg[j]);
             if (last) x[j] = R::mul(x[j], P.from_phase);
         }
     }

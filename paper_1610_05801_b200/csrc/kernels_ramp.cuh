@@ -191,7 +191,8 @@ __device__ __forceinline__ double ramp_kick(double v, double dl, const MapConsts
     double q = horner<double, R::NS>(P.sin1, s);
     if (HARM == 2) {
         const double cc = horner<double, R::NC>(P.cos1, s);
-        q = __dmul_rn(q, __fma_rn(R::flip_by(P.two_r, t), cc, 1.0));
+        q = __dmul_rn(q, __fma_rn(P.two_r, cc, R::sign_of(t)));      // one sign for sine and cosine (kick<> in kernels.cuh)
+        return __fma_rn(fa, q, base);
     }
     return __fma_rn(R::flip(fa, t), q, base);
 }
@@ -233,9 +234,11 @@ __device__ __forceinline__ void ramp_substep_scaled(double& u, double& y, const 
     double q = horner<double, R::NS>(P.sin1, s);
     if (HARM == 2) {
         const double cc = horner<double, R::NC>(P.cos1, s);
-        q = __dmul_rn(q, __fma_rn(R::flip_by(P.two_r, t), cc, 1.0));
+        q = __dmul_rn(q, __fma_rn(P.two_r, cc, R::sign_of(t)));
+        y = __fma_rn(f, q, base);
+    } else {
+        y = __fma_rn(R::flip(f, t), q, base);
     }
-    y = __fma_rn(R::flip(f, t), q, base);
     u = __fma_rn(-D, y, w);
 }
 
