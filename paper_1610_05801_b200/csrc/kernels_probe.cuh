@@ -30,6 +30,9 @@ probe_pipe_kernel(double* out, int iters, const __grid_constant__ ProbeConsts P,
     unsigned long long t0;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
     const unsigned long long c0 = clock64();
+    // the turn kinds are unrolled as deep as the kernel's own turn loop (LT_TURN_UNROLL particle-turns)
+    constexpr int kOuter = KIND >= 10 && LT_TURN_UNROLL / (8 * CHAINS) > 1 ? LT_TURN_UNROLL / (8 * CHAINS) : 1;
+#pragma unroll kOuter
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
