@@ -372,9 +372,9 @@ __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int 
         // every non-FP64 instruction costs issue capacity next to the saturated FP64 pipe
         // (profiles/r2_fp64_pipe_probe.md): the loop's 8 instructions of overhead (5 uniform-register
         // reloads, counter, compare, branch) are spread over LT_TURN_UNROLL particle-turns.  Configs[1]:
-        // 16 particle-turns per iteration 0.905 of the FP64 peak, 64: 0.912, 128: 0.915 -- and 256
-        // (57 KB of code): 0.59, the loop no longer fits the instruction cache; the default keeps a
-        // third of headroom below the largest body that measured well.  The double harmonic and
+        // 16 particle-turns per iteration 0.905 of the FP64 peak, 64: 0.912, 128: 0.915, 160: 0.911 --
+        // and 192 (43 KB of code): 0.858, 256 (57 KB): 0.59, the loop no longer fits the instruction
+        // cache; the default keeps a good third of headroom below the largest body that measured well.  The double harmonic and
         // Ruth4 measured BEST at 4 turns per iteration in fp64 (2: -2 points, 8: -1.5) and at 2 in the
         // packed fp32 kernels (0.864 of the FP32 peak against 0.845 at 4, 0.83 at 1 and 3).
 #ifndef LT_UNROLL_OTHER
