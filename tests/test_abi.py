@@ -93,6 +93,16 @@ def test_options_and_stats(lt):
         with pytest.raises(lt.LongtrackError) as e:
             tr.set_option(opt, bad)
         assert e.value.code == lt.E_PARAM
+    # round-2 options: defaults, round trip, range checks
+    assert tr.get_option(lt.OPT_RAMP_SCALED) == 1 and tr.get_option(lt.OPT_LATTICE_SOURCE) == 0
+    assert tr.get_option(lt.OPT_PER_TURN_CTAS_PER_SM) == 0          # planner
+    tr.set_option(lt.OPT_RAMP_SCALED, 0)
+    tr.set_option(lt.OPT_LATTICE_SOURCE, 2)
+    tr.set_option(lt.OPT_FUSED_ILP, 8)                              # fused transverse kernel only
+    assert (tr.get_option(lt.OPT_RAMP_SCALED), tr.get_option(lt.OPT_LATTICE_SOURCE), tr.get_option(lt.OPT_FUSED_ILP)) == (0, 2, 8)
+    for opt, bad in ((lt.OPT_LATTICE_SOURCE, 3), (lt.OPT_LATTICE_SOURCE, -1), (lt.OPT_FUSED_ILP, 16)):
+        with pytest.raises(lt.LongtrackError):
+            tr.set_option(opt, bad)
     assert tr.get_stat(lt.STAT_KERNEL_LAUNCHES) == 0
 
 
