@@ -669,11 +669,11 @@ __device__ __forceinline__ bool in_bucket(T z, T delta, const MapConsts<T>& P) {
 // Raw sums of a state, always accumulated in fp64.
 struct Sums {
     double sz, szz, sd, sdd, szd;
-    unsigned long long nin;
-    __device__ __forceinline__ void zero() { sz = szz = sd = sdd = szd = 0.0; nin = 0ULL; }
+    unsigned int nin;          // per THREAD: a thread sees at most n / (6 * 256) of the n <= 2^40 particles, < 2^32
+    __device__ __forceinline__ void zero() { sz = szz = sd = sdd = szd = 0.0; nin = 0u; }
     __device__ __forceinline__ void add(double z, double d, bool inb) {
         sz += z; szz = __fma_rn(z, z, szz); sd += d; sdd = __fma_rn(d, d, sdd);
-        szd = __fma_rn(z, d, szd); nin += inb ? 1ULL : 0ULL;
+        szd = __fma_rn(z, d, szd); nin += inb ? 1u : 0u;
     }
 };
 
@@ -787,7 +787,7 @@ __global__ void state_sums_kernel(const T* __restrict__ z_arr, const T* __restri
          i += (size_t)gridDim.x * blockDim.x) {
         T zz = z_arr[i], dd = d_arr[i];
         bool inb = in_bucket<T>(zz, dd, P);
-        if (ONLY_COUNT) acc.nin += inb ? 1ULL : 0ULL;
+        if (ONLY_COUNT) acc.nin += inb ? 1u : 0u;
         else acc.add((double)zz, (double)dd, inb);
     }
     block_reduce_store(acc, partials + (size_t)blockIdx.x * kPartialStride);
