@@ -76,7 +76,9 @@ enum {
                            (K_eff == 0 is allowed, G10)                         */
     LT_E_ALIGN    = -4, /* array pointer not aligned to its element size                  */
     LT_E_CUDA     = -5, /* a CUDA runtime call failed; see lt_last_cuda_error()           */
-    LT_E_NOMEM    = -6  /* host allocation failed                                         */
+    LT_E_NOMEM    = -6, /* host allocation failed                                         */
+    LT_E_CAPACITY = -7  /* n exceeds the fixed capacity of an entry point that works in the
+                           library's built-in scratch (lt_moments_now_static)             */
 };
 
 /* Ring / RF parameters: BASELINE.json:north_star (1) "(C, gamma, alpha_c, h, V, phi_s,
@@ -237,6 +239,45 @@ int lt_bucket_count_f32(lt_tracker *tr, const float *z_dev, const float *delta_d
 /* Moments of the current state (no tracking); either output may be NULL. */
 int lt_moments_now(lt_tracker *tr, const double *z_dev, const double *delta_dev, size_t n,
                    lt_moments *moments_dev, lt_sums *sums_dev, void *stream);
+
+/* lt_moments_now for callers that must not allocate device memory.
+ *
+ * Why it exists: lt_moments_now keeps its per-CTA partial sums in a tracker-owned buffer that
+ * its first call on a tracker (and any later call with a larger grid) takes from
+ * cudaMallocAsync.  Not every user of this library may do that -- a long-running tracking
+ * service that gives the whole GPU to its own memory pool at start-up leaves nothing for the
+ * driver's allocator; a turn-by-turn monitor at an interaction point must not
+ * stall on, or fail in, an allocation in the middle of a run; a plug-in inside somebody else's
+ * application may simply be forbidden to touch the CUDA heap.  This call computes the same
+ * observables (same predicate, same sums, fp64 accumulation; either output may be NULL, not
+ * both) and calls no cudaMalloc*, no cudaFree* and no library routine that allocates.
+ *
+ * How: the partial sums live in a fixed 128 KB array (`static __device__`, 256-byte aligned)
+ * that is part of the library image, one 64-byte record per 8192 particles.  Every GPU on which
+ * this library is loaded holds that array from load until the process exits, used or not.
+ *
+ * Limit: n <= LT_STATIC_MAX_PARTICLES (2^24 = 16 777 216, enough for BASELINE.json:configs[3]).
+ * A larger n returns LT_E_CAPACITY and enqueues nothing; use lt_moments_now there.
+ *
+ * Set-up: the FIRST call on each device asks the runtime once for the array's device address
+ * (cudaGetSymbolAddress, with that device current; a failure is LT_E_CUDA) and keeps it for
+ * the life of the process.  Make that first call during initialisation, before any stream
+ * capture is begun.  The current device must be the one z_dev / delta_dev live on, as for every
+ * other call; at most 64 devices per process (beyond that LT_E_PARAM).
+ *
+ * Sharing: there is ONE array per GPU for the whole process -- all trackers, all streams, all
+ * host threads.  It keeps what the previous call left in it; that is harmless, because each call
+ * writes every record it later reads and nothing has to start at zero.  But two calls whose
+ * kernels overlap on the same GPU (different streams, or different host threads on unordered
+ * streams) RACE on it and both results are garbage: order such calls on one stream or with
+ * events.  Calls on different GPUs do not interact.
+ *
+ * Results agree with lt_moments_now to rounding (the partition of the sum differs: ~1e-15
+ * relative on the sums); n_in_bucket is the same integer.  n == 0 writes all-zero outputs.
+ * Two launches on `stream`; asynchronous like every device call. */
+#define LT_STATIC_MAX_PARTICLES (1 << 24)
+int lt_moments_now_static(lt_tracker *tr, const double *z_dev, const double *delta_dev, size_t n,
+                          lt_moments *moments_dev, lt_sums *sums_dev, void *stream);
 
 /* Host helper: turns `count` raw sums (e.g. after an all-reduce over ranks) into moments. */
 int lt_moments_from_sums(const lt_sums *sums_host, size_t count, lt_moments *out_host);

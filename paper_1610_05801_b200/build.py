@@ -17,7 +17,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblongtrack.so")
 SOURCES = [os.path.join(CSRC, "longtrack.cu"), os.path.join(CSRC, "longtrack_next.cu"),
-           os.path.join(CSRC, "longtrack_ramp.cu")]
+           os.path.join(CSRC, "longtrack_ramp.cu"), os.path.join(CSRC, "longtrack_static.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "kernels_next.cuh"), os.path.join(CSRC, "kernels_ramp.cuh"), os.path.join(CSRC, "kernels_probe.cuh"),
                   os.path.join(CSRC, "tracker.hpp"), os.path.join(CSRC, "sinpi_coeffs.h"),
                   os.path.join(ROOT, "include", "longtrack.h")]

@@ -646,6 +646,7 @@ const char* lt_strerror(int code) {
         case LT_E_ALIGN: return "array pointer is not aligned to its element size";
         case LT_E_CUDA: return "CUDA runtime error (see lt_last_cuda_error)";
         case LT_E_NOMEM: return "out of host memory";
+        case LT_E_CAPACITY: return "n exceeds the fixed capacity of this no-allocation entry point (LT_STATIC_MAX_PARTICLES)";
         default: return "unknown error code";
     }
 }

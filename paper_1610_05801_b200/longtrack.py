@@ -24,6 +24,8 @@ EULER_CROMER, LEAPFROG, RUTH4 = 0, 1, 2
 INTEGRATORS = {"euler_cromer": EULER_CROMER, "leapfrog": LEAPFROG, "ruth4": RUTH4}
 
 OK, E_NULL, E_PARAM, E_UNSTABLE, E_ALIGN, E_CUDA, E_NOMEM = 0, -1, -2, -3, -4, -5, -6
+E_CAPACITY = -7
+STATIC_MAX_PARTICLES = 1 << 24    # lt_moments_now_static
 
 OPT_SPLIT_DRIFTS, OPT_CHUNK_TURNS, OPT_FUSED_ILP, OPT_FUSED_BLOCK = 1, 2, 3, 4
 OPT_PER_TURN_GRAPH, OPT_PER_TURN_CTAS_PER_SM, OPT_PER_TURN_REVERSE = 5, 6, 7
@@ -88,6 +90,7 @@ def _load():
         "lt_bucket_count": (c_int, [vp, vp, vp, sz, vp, vp]),
         "lt_bucket_count_f32": (c_int, [vp, vp, vp, sz, vp, vp]),
         "lt_moments_now": (c_int, [vp, vp, vp, sz, vp, vp, vp]),
+        "lt_moments_now_static": (c_int, [vp, vp, vp, sz, vp, vp, vp]),
         "lt_moments_from_sums": (c_int, [vp, sz, vp]),
         "lt_track_fused_host": (c_int, [vp, vp, vp, sz, ull, POINTER(ull)]),
         "lt_probe_fp64": (c_int, [c_int, c_int, c_int, c_longlong, POINTER(c_double),
@@ -215,6 +218,16 @@ class Tracker:
     def moments_now(self, z, delta, n: int, moments=None, sums=None, stream: int = 0):
         self._check(_lib.lt_moments_now(self._h, _ptr(z), _ptr(delta), n, _ptr(moments),
                                         _ptr(sums), stream))
+
+    def moments_now_static(self, z, delta, n: int, moments=None, sums=None, stream: int = 0):
+        """lt_moments_now without any device allocation, for callers that may not allocate (a
+        service whose own pool holds the whole GPU, a monitoring loop that must not stall or fail
+        in an allocation, a plug-in barred from the CUDA heap): partial sums go to a fixed 128 KB
+        array built into the library.  n <= STATIC_MAX_PARTICLES, else E_CAPACITY.  The array is
+        shared by the whole process: calls that overlap on one GPU race.  First call per device
+        looks the array up; make it before any stream capture."""
+        self._check(_lib.lt_moments_now_static(self._h, _ptr(z), _ptr(delta), n, _ptr(moments),
+                                               _ptr(sums), stream))
 
     # ---- SURVEY.md sec. 8(f) rows f2-f4 (device pointers; tables are device arrays too)
     def track_programme(self, z, delta, n: int, turns: int, volt_scale, phase_off,
