@@ -159,7 +159,10 @@ enum {
                                   again and again); results do not depend on it                    */
     LT_OPT_WARPS_PER_SMSP = 10,/* resident warps per SM sub-partition of the persistent kernel
                                   (0 = planner; 1..8, or even values up to 16; with two particles
-                                  per lane at most 4)                                               */
+                                  per lane at most 4).  Forced options that admit no launch shape
+                                  together are given up in a fixed order -- FUSED_MODE 4 -> 2, then
+                                  FUSED_ILP 2 -> planner (the warp count is kept), then all of them
+                                  -- and LT_STAT_LAST_* report what was launched                    */
     LT_OPT_FLIP_ON_Q      = 11,/* where the sign of the reduced sine is applied: -1 planner,
                                   0 on the argument, 1 on the polynomial; same bits either way */
     LT_OPT_RAMP_SCALED    = 12,/* lt_track_ramp, merged drifts: 1 (default) carries delta divided by

@@ -227,7 +227,8 @@ double loop_rate(int ilp, int w, bool fq) {
 
 }  // namespace
 namespace lt_host {
-PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns, int max_ilp, int pv) {
+// The best launch shape that the tracker's forced options allow; false when they allow none.
+static bool search_persistent(const lt_tracker* tr, size_t n, int max_ilp, int pv, PersistentPlan* out) {
     const int sms = tr->sm_count;
     PersistentPlan best = {0, 4, 1, 512, 0, false, 1};
     double best_score = -1.0;
@@ -281,10 +282,34 @@ PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long lon
             }
         }
     }
-    if (best_score < 0.0) {                                  // forced wrap-around with fewer groups than slots
+    *out = best;
+    return best_score >= 0.0;
+}
+
+PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns, int max_ilp, int pv) {
+    PersistentPlan best = {0, 4, 1, 512, 0, false, 1};
+    if (!search_persistent(tr, n, max_ilp, pv, &best)) {
+        // The forced options (each valid on its own, include/longtrack.h) admit no launch shape
+        // together.  Give them up one at a time, the least binding first -- a fixed, finite list,
+        // so the planner always returns; what was actually launched is in LT_STAT_LAST_*.
         lt_tracker relaxed = *tr;
-        relaxed.fused_mode = 2;
-        return plan_persistent(&relaxed, n, turns, max_ilp, pv);
+        bool found = false;
+        if (relaxed.fused_mode == 4) {                       // wrap-around with fewer groups than slots
+            relaxed.fused_mode = 2;
+            found = search_persistent(&relaxed, n, max_ilp, pv, &best);
+        }
+        if (!found && relaxed.fused_ilp == 2) {              // two particles per lane exist up to 4 warps
+            relaxed.fused_ilp = 0;                           // per sub-partition only: keep the warp count
+            found = search_persistent(&relaxed, n, max_ilp, pv, &best);
+        }
+        if (!found) {
+            relaxed.fused_mode = 0;
+            relaxed.warps_per_smsp = 0;
+            relaxed.flip_on_q = -1;
+            relaxed.fused_ilp = 0;
+            found = search_persistent(&relaxed, n, max_ilp, pv, &best);
+        }
+        if (!found) best = PersistentPlan{0, 4, 1, 512, 0, false, 1};   // n == 0: nothing to place
     }
     if (best.dynamic == 1) {
         // an item switch costs a warp about 3 us (ticket, progress word, state load; store, fence,

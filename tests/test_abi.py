@@ -270,3 +270,45 @@ def test_planner_picks_the_measured_launch_shapes(lt):
     assert p["threads"] == 640
     with pytest.raises(lt.LongtrackError):
         tr.plan_fused(0, 10)
+
+
+def test_planner_returns_for_every_combination_of_forced_options(lt):
+    """Each option value is valid on its own; no combination may hang or crash the planner
+    (FUSED_ILP = 2 with more than 4 warps per sub-partition used to recurse without end).  A
+    combination that no launch shape honours gives up ILP 2 first and keeps the warp count."""
+    from paper_1610_05801_b200 import workloads as wl
+    tr = lt.Tracker(wl.RING, "leapfrog")
+    warps = [0, 1, 2, 3, 4, 5, 6, 7, 8, 10, 12, 14, 16]
+    for n in (1, 63, 1_000, 100_000, 1_000_003):
+        for fp32 in (False, True):
+            for ilp in (0, 1, 2):
+                for w in warps:
+                    for mode in (lt.FUSED_AUTO, lt.FUSED_PERSISTENT_STATIC,
+                                 lt.FUSED_PERSISTENT_DYNAMIC, lt.FUSED_PERSISTENT_WRAP):
+                        for fq in (-1, 0, 1):
+                            tr.set_option(lt.OPT_FUSED_ILP, ilp)
+                            tr.set_option(lt.OPT_WARPS_PER_SMSP, w)
+                            tr.set_option(lt.OPT_FUSED_MODE, mode)
+                            tr.set_option(lt.OPT_FLIP_ON_Q, fq)
+                            p = tr.plan_fused(n, 1000, fp32=fp32)
+                            pv = 2 if fp32 else 1
+                            assert p["particles_per_lane"] in (pv, 2 * pv)
+                            assert p["threads"] * p["ctas_per_sm"] == 128 * p["warps_per_smsp"]
+                            assert 32 <= p["threads"] <= 1024 and p["ctas_per_sm"] in (1, 2)
+                            if w:
+                                assert p["warps_per_smsp"] == w
+                            if w > 4:
+                                assert p["particles_per_lane"] == pv     # ILP 2 given up, W kept
+                            elif ilp:
+                                assert p["particles_per_lane"] == ilp * pv
+                            if fq >= 0:
+                                assert p["flip_on_q"] == fq
+                            if mode == lt.FUSED_PERSISTENT_STATIC:
+                                assert p["dynamic"] == 0
+                            if mode == lt.FUSED_PERSISTENT_DYNAMIC:
+                                assert p["dynamic"] == 1
+    tr.set_option(lt.OPT_FUSED_ILP, 2)
+    tr.set_option(lt.OPT_WARPS_PER_SMSP, 8)
+    tr.set_option(lt.OPT_FUSED_MODE, lt.FUSED_AUTO)
+    p = tr.plan_fused(100_000, 70_000)                       # the advisor's reproducer (ADVICE r2)
+    assert (p["particles_per_lane"], p["warps_per_smsp"], p["threads"]) == (1, 8, 1024)
