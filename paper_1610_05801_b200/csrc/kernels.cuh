@@ -66,6 +66,7 @@ template <> struct Real<double> {
     static __device__ __forceinline__ double add(double a, double b) { return __dadd_rn(a, b); }
     static __device__ __forceinline__ double sub(double a, double b) { return __dsub_rn(a, b); }
     static __device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
+    static __device__ __forceinline__ double mul_rounded(double a, double b) { return __dmul_rn(a, b); }   // see Real<f32x2>
     // f with the sign bit flipped when the integer held in the low mantissa bits of t is odd.
     // hi + (lo << 31) mod 2^32 == hi ^ ((lo & 1) << 31): ONE IMAD instead of shift + xor, in
     // unsigned arithmetic (defined on overflow).  Next to a saturated FP64 pipe the IMAD costs
@@ -94,6 +95,7 @@ template <> struct Real<float> {
     static __device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b); }
     static __device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
     static __device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
+    static __device__ __forceinline__ float mul_rounded(float a, float b) { return __fmul_rn(a, b); }     // see Real<f32x2>
     static __device__ __forceinline__ float flip(float f, float t) {
         return __uint_as_float(__float_as_uint(f) + (__float_as_uint(t) << 31));
     }
@@ -126,6 +128,16 @@ template <> struct Real<f32x2> {
     static __device__ __forceinline__ f32x2 add(f32x2 a, f32x2 b) { return wrap(__fadd2_rn(a.v, b.v)); }
     static __device__ __forceinline__ f32x2 sub(f32x2 a, f32x2 b) { return wrap(__fadd2_rn(a.v, (-b).v)); }
     static __device__ __forceinline__ f32x2 mul(f32x2 a, f32x2 b) { return wrap(__fmul2_rn(a.v, b.v)); }
+    // A product that feeds an ADDITION and has to keep its own rounding (the phase v = z * kappa/pi
+    // of the exact path, which the reduction adds to and subtracts from).  ptxas 12.9 contracts
+    // mul.rn.f32x2 + add.rn.f32x2 into one FFMA2 in spite of the explicit roundings -- also with
+    // --fmad=false, also when the product is written fma(a, b, -0) -- which it never does to the
+    // scalar mul.rn.f32 / mul.rn.f64; the packed kernels then returned other bits than the scalar
+    // fp32 kernels (plain fused, per-turn) on the split-drift path.  Two scalar FMULs are left
+    // alone (checked in the SASS); they cost one issue slot more, on the exact path only.
+    static __device__ __forceinline__ f32x2 mul_rounded(f32x2 a, f32x2 b) {
+        return f32x2(__fmul_rn(a.v.x, b.v.x), __fmul_rn(a.v.y, b.v.y));
+    }
     // With packed arithmetic the FMA pipe is the bound (two cycles per FFMA2) and issue slots are
     // free, so the sign flip leaves that pipe: funnel shift + XOR on the ALU pipe instead of the
     // IMAD of the scalar kernels (an IMAD occupies the FMA pipe; profiles/r2_ncu_summary.md).
@@ -224,7 +236,7 @@ __device__ __forceinline__ T kick(T v, T delta, const MapConsts<T>& P, int stage
         T t1, t2;
         T f1 = reduce_half_periods(R::add(v, P.phi_off), &t1);
         T s1 = R::mul(f1, f1);
-        T sn = R::mul(R::flip(f1, t1), horner<T, NS>(P.sin1, s1));
+        T sn = R::mul_rounded(R::flip(f1, t1), horner<T, NS>(P.sin1, s1));   // feeds a subtraction
         T acc = R::sub(sn, P.sin_phi_s);
         T f2 = reduce_half_periods(R::add(v, v), &t2);
         T s2 = R::mul(f2, f2);
@@ -243,7 +255,7 @@ __device__ __forceinline__ void turn_exact(T& z, T& delta, const MapConsts<T>& P
                                            T p = T(0)) {
     typedef Real<T> R;
     constexpr int PK = PROG ? 2 : 0;
-#define LT_PHASE(zz) (PROG ? R::fma(zz, P.to_phase, p) : R::mul(zz, P.to_phase))
+#define LT_PHASE(zz) (PROG ? R::fma(zz, P.to_phase, p) : R::mul_rounded(zz, P.to_phase))
     if (INTEG == kLeapfrog) {
         z = R::fma(-P.zdrift_lead, delta, z);
         delta = kick<T, HARM, false, PK>(LT_PHASE(z), delta, P, 0, a);
@@ -365,7 +377,7 @@ __device__ __forceinline__ void advance(T (&x)[ILP], T (&dl)[ILP], unsigned int 
         if (first) {
 #pragma unroll
             for (int j = 0; j < ILP; ++j) {
-                x[j] = R::mul(x[j], P.to_phase);
+                x[j] = R::mul_rounded(x[j], P.to_phase);     // Euler-Cromer: goes straight into the reduction
                 if (INTEG != kEulerCromer) x[j] = R::fma(-P.drift_lead, dl[j], x[j]);
             }
         }
