@@ -884,8 +884,7 @@ def main():
         entry.build()
     else:                                               # torchrun: local rank 0 builds, the others wait
         from paper_1610_05801_b200 import build as lt_build
-        lt_build.wait_until_built()
-        time.sleep(1.0)                                 # let the linker finish writing
+        lt_build.wait_until_built()                     # the library appears by an atomic rename
     run_cuda(args)
 
 

@@ -37,11 +37,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     newest = max(os.path.getmtime(p) for p in DEPS)
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
-    cmd = [nvcc(), *NVCC_FLAGS, "-o", LIB, *SOURCES]
+    # nvcc/ld write their output in place: link to a private name and rename it onto LIB, so that
+    # another process (the non-zero ranks of a torchrun launch, wait_until_built below) can never
+    # dlopen a half-written library -- os.replace is atomic within one directory
+    tmp = "%s.tmp.%d" % (LIB, os.getpid())
+    cmd = [nvcc(), *NVCC_FLAGS, "-o", tmp, *SOURCES]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd))
-    subprocess.run(cmd, check=True, cwd=HERE)
+    try:
+        subprocess.run(cmd, check=True, cwd=HERE)
+        os.replace(tmp, LIB)
+    finally:
+        if os.path.exists(tmp):
+            os.remove(tmp)
     return LIB
 
 

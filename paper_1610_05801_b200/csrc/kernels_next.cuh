@@ -200,17 +200,23 @@ static __global__ void advance_cursor_kernel(unsigned long long* cursor, unsigne
 // after the previous tile's atomics and ran 1184 short-lived CTAs whose zero / load / flush
 // phases coincided: 3.7 TB/s in the kernel, profiles/r1_next_rows_ncu.md).
 // No memset launch and no serial tail: CTA 0 zeroes the caller's histogram while its first tile is
-// in flight and then publishes the call's `epoch` in *flag (release); every CTA streams its
-// share into its shared-memory copies and, ~15 us later, adds them to the caller's histogram
-// after an acquire-read of the flag (CTA 0 is the first CTA the hardware dispatches, so the flag
-// is never actually waited on).  Round 2's first version summed into a tracker-owned accumulator
+// in flight and then sets flag[0] = 1 (release); every CTA streams its share into its
+// shared-memory copies and, ~15 us later, adds them to the caller's histogram after an
+// acquire-read of flag[0] (CTA 0 is normally the first CTA dispatched, so the flag is hardly ever
+// waited on; correctness does not rest on that -- the grid is one wave, CTA 0 is resident).
+// The protocol's state lives on the DEVICE only: each CTA signs off in flag[1] once it is past the
+// wait, and the last one to do so puts both words back to 0, which is what the next launch --
+// stream-ordered behind this one -- starts from.  No per-call value comes from the host, so a
+// launch replayed from a CUDA graph behaves like a fresh call (round 2 passed a host-side call
+// number as a kernel argument, which a replay would have repeated).
+// Round 2's first version summed into a tracker-owned accumulator
 // that the LAST CTA copied out: a serial fence + ticket + copy behind the slowest CTA.
 // flag == nullptr: the caller zeroed `out` (more slices than the shared-memory path holds).
 // A z array that is only 8-byte aligned is shifted by one element (`head`).
 template <int UNR>
 static __global__ void __launch_bounds__(512)
 slice_histogram_kernel(const double* __restrict__ z_arr, size_t n, const __grid_constant__ TurnExtras X,
-                       unsigned int* __restrict__ flag, unsigned int epoch) {
+                       unsigned int* __restrict__ flag) {
     extern __shared__ unsigned int slice_smem[];
     const size_t head = ((reinterpret_cast<uintptr_t>(z_arr) & 15u) != 0 && n > 0) ? 1 : 0;
     const double* __restrict__ zb = z_arr + head;
@@ -229,7 +235,7 @@ slice_histogram_kernel(const double* __restrict__ z_arr, size_t n, const __grid_
         for (int b = threadIdx.x; b < X.n_slices + 2; b += blockDim.x) X.hist[b] = 0ULL;
         __threadfence();
         __syncthreads();
-        if (threadIdx.x == 0) st_release_u32(flag, epoch);
+        if (threadIdx.x == 0) st_release_u32(flag, 1u);
     }
     SliceAcc sl;
     sl.init(X, 0ULL, slice_smem);
@@ -254,9 +260,14 @@ slice_histogram_kernel(const double* __restrict__ z_arr, size_t n, const __grid_
     for (size_t i = base + threadIdx.x; i < m && base < m; i += blockDim.x) {
         if (i < base + tile) sl.add(zb[i]);
     }
-    if (flag && blockIdx.x != 0) {            // the histogram has been zeroed for THIS call
-        if (threadIdx.x == 0) {
-            while (ld_acquire_u32(flag) != epoch) __nanosleep(32);
+    if (flag && threadIdx.x == 0) {
+        if (blockIdx.x != 0) {                // the histogram has been zeroed by THIS launch
+            while (ld_acquire_u32(flag) != 1u) __nanosleep(32);
+        }
+        // past the wait: sign off; the last CTA to do so re-arms both words for the next launch
+        if (atomicAdd(flag + 1, 1u) == gridDim.x - 1) {
+            flag[1] = 0u;
+            st_release_u32(flag, 0u);
         }
         // SliceAcc::flush starts with a __syncthreads(), which orders every thread behind the acquire
     }

@@ -230,7 +230,7 @@ namespace lt_host {
 // The best launch shape that the tracker's forced options allow; false when they allow none.
 static bool search_persistent(const lt_tracker* tr, size_t n, int max_ilp, int pv, PersistentPlan* out) {
     const int sms = tr->sm_count;
-    PersistentPlan best = {0, 4, 1, 512, 0, false, 1};
+    PersistentPlan best = {0, 4, 1, 512, 0, false, 1, 1};
     double best_score = -1.0;
     for (int ilp = 1; ilp <= max_ilp; ++ilp) {
         if (max_ilp > 1 && (tr->fused_ilp == 1 || tr->fused_ilp == 2) && ilp != tr->fused_ilp) continue;
@@ -287,7 +287,7 @@ static bool search_persistent(const lt_tracker* tr, size_t n, int max_ilp, int p
 }
 
 PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long long turns, int max_ilp, int pv) {
-    PersistentPlan best = {0, 4, 1, 512, 0, false, 1};
+    PersistentPlan best = {0, 4, 1, 512, 0, false, 1, 1};
     if (!search_persistent(tr, n, max_ilp, pv, &best)) {
         // The forced options (each valid on its own, include/longtrack.h) admit no launch shape
         // together.  Give them up one at a time, the least binding first -- a fixed, finite list,
@@ -309,20 +309,17 @@ PersistentPlan plan_persistent(const lt_tracker* tr, size_t n, unsigned long lon
             relaxed.fused_ilp = 0;
             found = search_persistent(&relaxed, n, max_ilp, pv, &best);
         }
-        if (!found) best = PersistentPlan{0, 4, 1, 512, 0, false, 1};   // n == 0: nothing to place
+        if (!found) best = PersistentPlan{0, 4, 1, 512, 0, false, 1, 1};   // n == 0: nothing to place
     }
-    if (best.dynamic == 1) {
-        // an item switch costs a warp about 3 us (ticket, progress word, state load; store, fence,
-        // release), during which its sub-partition runs at half rate when it holds two warps: long
-        // items (2048 turns = 120 us) amortise that, and the tapered tail of the schedule
-        // (ItemSchedule) keeps the last round short all the same (profiles/r2_fused_shapes.md)
-        unsigned long long it = tr->item_turns > 0
-                                    ? (unsigned long long)tr->item_turns
-                                    : std::min<unsigned long long>(2048, std::max<unsigned long long>(128, turns / 8));
-        best.item_turns = (unsigned int)std::min<unsigned long long>(it, turns);
-    } else {
-        best.item_turns = 0;                                 // = all turns of the launch
-    }
+    // an item switch costs a warp about 3 us (ticket, progress word, state load; store, fence,
+    // release), during which its sub-partition runs at half rate when it holds two warps: long
+    // items (2048 turns = 120 us) amortise that, and the tapered tail of the schedule
+    // (ItemSchedule) keeps the last round short all the same (profiles/r2_fused_shapes.md)
+    unsigned long long it = tr->item_turns > 0
+                                ? (unsigned long long)tr->item_turns
+                                : std::min<unsigned long long>(2048, std::max<unsigned long long>(128, turns / 8));
+    best.queue_item_turns = (unsigned int)std::max<unsigned long long>(1, std::min<unsigned long long>(it, turns));
+    best.item_turns = best.dynamic == 1 ? best.queue_item_turns : 0;   // 0 = all turns of the launch
     return best;
 }
 }  // namespace lt_host
@@ -340,14 +337,24 @@ cudaError_t launch_persistent_ilp(T* z, T* d, size_t n, unsigned int turns, unsi
     auto kern = fused_persistent_kernel<T, INTEG, HARM, SPLIT, FQ, false, ILP, typename ChainValue<T>::type>;
     // 1 CTA/SM: > half of the 227 KB; 2 CTAs/SM: > a third
     const int smem = pl.ctas_per_sm == 1 ? 120 * 1024 : 80 * 1024;
-    static bool attr_set = false;                            // once per instantiation
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+    static std::atomic<unsigned long long> attr_devices{0};   // per instantiation: the devices it is set on
+    {
+        cudaError_t e = allow_dynamic_smem(attr_devices, kern, 120 * 1024);
         if (e != cudaSuccess) return e;
-        attr_set = true;
     }
-    kern<<<sms * pl.ctas_per_sm, pl.threads, smem, st>>>(z, d, n, turns, item_turns, first, last, pl.dynamic, sched,
-                                      reinterpret_cast<unsigned int*>(sched + 1), c, nullptr);
+    unsigned int* const done = reinterpret_cast<unsigned int*>(sched + 1);
+    int dynamic = pl.dynamic;
+    if (dynamic == 2) {                                      // CTAs wait on one another: co-resident or not at all
+        const cudaError_t e = launch_coresident(kern, sms * pl.ctas_per_sm, pl.threads, (size_t)smem, st, z, d, n,
+                                                turns, item_turns, first, last, 2, sched, done, c, nullptr);
+        if (!coresidency_refused(e)) return e;
+        (void)cudaGetLastError();
+        g_wrap_refused = 1;                                  // same bits from the ticket queue
+        dynamic = 1;
+        item_turns = std::min(pl.queue_item_turns, turns);
+    }
+    kern<<<sms * pl.ctas_per_sm, pl.threads, smem, st>>>(z, d, n, turns, item_turns, first, last, dynamic, sched,
+                                                         done, c, nullptr);
     return cudaGetLastError();
 }
 
@@ -401,6 +408,7 @@ int track_fused_persistent(lt_tracker* tr, T* z, T* d, size_t n, unsigned long l
     if (rc) return rc;
     unsigned long long done = 0;
     PersistentPlan pl = plan_persistent(tr, n, turns, 2, kPV);
+    g_wrap_refused = 0;
     while (done < turns) {
         unsigned long long chunk = std::min<unsigned long long>(turns - done, (unsigned long long)tr->chunk_turns);
         const int first = done == 0, last = done + chunk == turns;
@@ -429,8 +437,8 @@ int track_fused_persistent(lt_tracker* tr, T* z, T* d, size_t n, unsigned long l
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
     tr->last_ilp = pl.ilp * kPV;
-    tr->last_mode = pl.dynamic == 2 ? 4 : (pl.dynamic ? 3 : 2);
-    tr->last_item_turns = pl.dynamic == 1 ? pl.item_turns : 0;
+    tr->last_mode = pl.dynamic == 2 ? (g_wrap_refused ? 3 : 4) : (pl.dynamic ? 3 : 2);
+    tr->last_item_turns = pl.dynamic == 1 ? pl.item_turns : (pl.dynamic == 2 && g_wrap_refused ? pl.queue_item_turns : 0);
     return LT_OK;
 }
 

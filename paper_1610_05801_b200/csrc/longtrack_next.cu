@@ -33,15 +33,24 @@ cudaError_t launch_prog_ilp(double* z, double* d, size_t n, unsigned int turns, 
                             const double2* prog, cudaStream_t st) {
     auto kern = fused_persistent_kernel<double, INTEG, HARM, SPLIT, FQ, true, ILP>;
     const int smem = residency_smem(pl);                     // >= 512 B of staged entries per warp
-    static bool attr_set = false;                            // once per instantiation
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+    static std::atomic<unsigned long long> attr_devices{0};   // per instantiation: the devices it is set on
+    {
+        cudaError_t e = allow_dynamic_smem(attr_devices, kern, 120 * 1024);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+    }
+    unsigned int* const done = reinterpret_cast<unsigned int*>(sched + 1);
+    int dynamic = pl.dynamic;
+    if (dynamic == 2) {                                      // CTAs wait on one another: co-resident or not at all
+        const cudaError_t e = launch_coresident(kern, sms * pl.ctas_per_sm, pl.threads, (size_t)smem, st, z, d, n,
+                                                turns, item_turns, first, last, 2, sched, done, c, prog);
+        if (!coresidency_refused(e)) return e;
+        (void)cudaGetLastError();
+        g_wrap_refused = 1;                                  // same bits from the ticket queue
+        dynamic = 1;
+        item_turns = std::min(pl.queue_item_turns, turns);
     }
     kern<<<sms * pl.ctas_per_sm, pl.threads, smem, st>>>(z, d, n, turns, item_turns, first, last,
-                                                         pl.dynamic, sched,
-                                                         reinterpret_cast<unsigned int*>(sched + 1), c, prog);
+                                                         dynamic, sched, done, c, prog);
     return cudaGetLastError();
 }
 
@@ -91,6 +100,7 @@ int track_programme_fused(lt_tracker* tr, double* z, double* d, size_t n, unsign
         if (tr->prog_entries < want) tr->prog_entries = want;
     }
     const PersistentPlan pl = plan_persistent(tr, n, turns, 2);
+    g_wrap_refused = 0;
     unsigned long long done = 0;
     while (done < turns) {
         const unsigned long long chunk = std::min<unsigned long long>(turns - done, chunk_max);
@@ -120,8 +130,8 @@ int track_programme_fused(lt_tracker* tr, double* z, double* d, size_t n, unsign
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
     tr->last_ilp = pl.ilp;
-    tr->last_mode = pl.dynamic == 2 ? 4 : (pl.dynamic ? 3 : 2);
-    tr->last_item_turns = pl.dynamic == 1 ? pl.item_turns : 0;
+    tr->last_mode = pl.dynamic == 2 ? (g_wrap_refused ? 3 : 4) : (pl.dynamic ? 3 : 2);
+    tr->last_item_turns = pl.dynamic == 1 ? pl.item_turns : (pl.dynamic == 2 && g_wrap_refused ? pl.queue_item_turns : 0);
     return LT_OK;
 }
 
@@ -357,11 +367,10 @@ cudaError_t launch_transverse_one(double* x, double* xp, double* y, double* yp, 
                                   const PersistentPlan& pl, const lt_tracker* tr, cudaStream_t st) {
     auto kern = transverse_persistent_kernel<NSEG, LONGI, ILP>;
     const int smem = residency_smem(pl);                 // >= the lattice (256 x 128 B)
-    static bool attr_set = false;                        // once per instantiation
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+    static std::atomic<unsigned long long> attr_devices{0};   // per instantiation: the devices it is set on
+    {
+        cudaError_t e = allow_dynamic_smem(attr_devices, kern, 120 * 1024);
         if (e != cudaSuccess) return e;
-        attr_set = true;
     }
     kern<<<tr->sm_count * pl.ctas_per_sm, pl.threads, smem, st>>>(
         x, xp, y, yp, z, d, n, turns, item_turns, first, last, pl.dynamic, tr->sched,
@@ -376,11 +385,10 @@ cudaError_t launch_transverse_param(double* x, double* xp, double* y, double* yp
                                     const PersistentPlan& pl, const lt_tracker* tr, cudaStream_t st) {
     auto kern = transverse_persistent_param_kernel<LONGI, ILP>;
     const int smem = residency_smem(pl);
-    static bool attr_set = false;                        // once per instantiation
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+    static std::atomic<unsigned long long> attr_devices{0};   // per instantiation: the devices it is set on
+    {
+        cudaError_t e = allow_dynamic_smem(attr_devices, kern, 120 * 1024);
         if (e != cudaSuccess) return e;
-        attr_set = true;
     }
     LatticeParam lp;
     std::memcpy(lp.m, tr->lattice_host, (size_t)tr->n_seg * 16 * sizeof(double));
@@ -577,8 +585,8 @@ int lt_slice_histogram(lt_tracker* tr, const double* z_dev, size_t n, double z_l
         LT_CUDA(tr, cudaMemsetAsync(hist_dev, 0, ((size_t)n_slices + 2) * sizeof(unsigned long long), st));
         if (n == 0) return LT_OK;
     } else if (!tr->hist_acc) {
-        // the epoch flag of the shared-memory path: CTA 0 publishes "the histogram of call number
-        // hist_epoch has been zeroed" in it
+        // the two words of the shared-memory path's protocol ("zeroed" flag, sign-off count): both 0
+        // between launches, the kernel itself puts them back
         LT_CUDA(tr, cudaMallocAsync((void**)&tr->hist_acc, sizeof(unsigned long long), st));
         LT_CUDA(tr, cudaMemsetAsync(tr->hist_acc, 0, sizeof(unsigned long long), st));
     }
@@ -588,9 +596,8 @@ int lt_slice_histogram(lt_tracker* tr, const double* z_dev, size_t n, double z_l
     // one wave: as many CTAs as are resident together (the flag protocol of the kernel needs CTA 0
     // running while the others wait for it; it is the first one dispatched)
     g = std::max<size_t>(1, std::min<size_t>(g, (size_t)tr->sm_count * 2));   // 3 per SM measured the same
-    if (!direct && ++tr->hist_epoch == 0u) tr->hist_epoch = 1u;   // 0 is the flag's initial value
     slice_histogram_kernel<kUnr><<<(unsigned)g, kThreads, smem, st>>>(
-        z_dev, n, X, direct ? nullptr : reinterpret_cast<unsigned int*>(tr->hist_acc), tr->hist_epoch);
+        z_dev, n, X, direct ? nullptr : reinterpret_cast<unsigned int*>(tr->hist_acc));
     LT_CUDA(tr, cudaGetLastError());
     tr->launches++;
     return LT_OK;

@@ -71,17 +71,27 @@ cudaError_t launch_ramp_fused_ilp(double* z, double* d, size_t n, unsigned int n
     // holds 3072 B of staging per warp: 32 warps of a 2-CTA launch need 96 KB, which still fits twice
     const int warps = pl.threads / 32;
     const int smem = std::max(pl.ctas_per_sm == 1 ? 120 * 1024 : 80 * 1024, warps * 3072);
-    static bool attr_set = false;                            // once per instantiation
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 120 * 1024);
+    static std::atomic<unsigned long long> attr_devices{0};   // per instantiation: the devices it is set on
+    {
+        cudaError_t e = allow_dynamic_smem(attr_devices, kern, 120 * 1024);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+    }
+    unsigned int* const done = reinterpret_cast<unsigned int*>(tr->sched + 1);
+    const double2* const table = SCALED ? reinterpret_cast<const double2*>(scaled_table(tr))
+                                        : reinterpret_cast<const double2*>(tr->ramp_table);
+    int dynamic = pl.dynamic;
+    if (dynamic == 2) {                                      // CTAs wait on one another: co-resident or not at all
+        const cudaError_t e = launch_coresident(kern, tr->sm_count * pl.ctas_per_sm, pl.threads, (size_t)smem, st,
+                                                z, d, n, nsteps, item_steps, first, last, 2, tr->sched, done,
+                                                tr->c64, table, flag);
+        if (!coresidency_refused(e)) return e;
+        (void)cudaGetLastError();
+        g_wrap_refused = 1;                                  // same bits from the ticket queue
+        dynamic = 1;
+        item_steps = std::min(pl.queue_item_turns * (unsigned int)nsub_of(tr), nsteps);
     }
     kern<<<tr->sm_count * pl.ctas_per_sm, pl.threads, smem, st>>>(
-        z, d, n, nsteps, item_steps, first, last, pl.dynamic, tr->sched,
-        reinterpret_cast<unsigned int*>(tr->sched + 1), tr->c64,
-        SCALED ? reinterpret_cast<const double2*>(scaled_table(tr)) : reinterpret_cast<const double2*>(tr->ramp_table),
-        flag);
+        z, d, n, nsteps, item_steps, first, last, dynamic, tr->sched, done, tr->c64, table, flag);
     return cudaGetLastError();
 }
 
@@ -173,6 +183,7 @@ int lt_track_ramp(lt_tracker* tr, double* z, double* d, size_t n, unsigned long 
     rc = ensure_ramp_table(tr, (size_t)std::min<unsigned long long>(turns, chunk_max) * nsub + 1, st);   // + header
     if (rc) return rc;
     const PersistentPlan pl = plan_persistent(tr, n, turns, 2);
+    g_wrap_refused = 0;
     const RampRing R = make_ring(tr);
     // which fast layout: the scaled one divides by the kick amplitude tau a_t A(p) of every sub-step
     int layout = 0;
@@ -213,8 +224,8 @@ int lt_track_ramp(lt_tracker* tr, double* z, double* d, size_t n, unsigned long 
     tr->last_grid = (long long)tr->sm_count * pl.ctas_per_sm;
     tr->last_block = pl.threads;
     tr->last_ilp = pl.ilp;
-    tr->last_mode = pl.dynamic == 2 ? 4 : (pl.dynamic ? 3 : 2);
-    tr->last_item_turns = pl.dynamic == 1 ? pl.item_turns : 0;
+    tr->last_mode = pl.dynamic == 2 ? (g_wrap_refused ? 3 : 4) : (pl.dynamic ? 3 : 2);
+    tr->last_item_turns = pl.dynamic == 1 ? pl.item_turns : (pl.dynamic == 2 && g_wrap_refused ? pl.queue_item_turns : 0);
     return LT_OK;
 }
 

@@ -5,7 +5,10 @@
 
 #include "../../include/longtrack.h"
 
+#include <atomic>
 #include <cstdint>
+#include <tuple>
+#include <utility>
 #include <cuda_runtime.h>
 
 #include "kernels.cuh"
@@ -43,6 +46,8 @@ struct PersistentPlan {
     unsigned int item_turns;
     bool flip_on_q;
     int ilp;                  // particles per lane of the persistent kernel (1 or 2)
+    unsigned int queue_item_turns;   // item length the ticket queue would use (always set): what a
+                                     // refused wrap-around launch falls back to
 };
 
 }  // namespace lt_host
@@ -79,9 +84,8 @@ struct lt_tracker {
     // f2: packed programme table of the current fused chunk
     double2* prog_table;
     size_t prog_entries;
-    // f4: epoch flag of lt_slice_histogram ("the caller's histogram has been zeroed for call hist_epoch")
+    // f4: the two protocol words of lt_slice_histogram ("zeroed" flag, sign-off count), 0 between launches
     unsigned long long* hist_acc;
-    unsigned int hist_epoch;
     // f2 with acceleration: packed sub-step entries (lt::RampEntry, 48 B each)
     void* ramp_table;
     size_t ramp_entries;
@@ -106,21 +110,73 @@ namespace lt_host {
 inline bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
 
 // Grows a tracker-owned device buffer to `need` bytes, STREAM-ORDERED on the caller's stream
-// (cudaFreeAsync + cudaMallocAsync): no device synchronisation, unlike cudaFree/cudaMalloc.  The
+// (cudaMallocAsync + cudaFreeAsync): no device synchronisation, unlike cudaFree/cudaMalloc.  The
 // old block is released after the work already enqueued on `st`, the new one is usable by what
 // is enqueued after this call (one call in flight per tracker: include/longtrack.h).
+// The new block is obtained FIRST: when that fails, *ptr and *have -- and with them whatever
+// capacity the tracker derives from *have -- still describe the old block, which stays usable.
 inline cudaError_t grow_async(void** ptr, size_t* have, size_t need, cudaStream_t st) {
     if (*have >= need && *ptr) return cudaSuccess;
+    void* fresh = nullptr;
+    cudaError_t e = cudaMallocAsync(&fresh, need, st);
+    if (e != cudaSuccess) return e;
     if (*ptr) {
-        cudaError_t e = cudaFreeAsync(*ptr, st);
-        if (e != cudaSuccess) return e;
-        *ptr = nullptr;
-        *have = 0;
+        e = cudaFreeAsync(*ptr, st);
+        if (e != cudaSuccess) {
+            (void)cudaFreeAsync(fresh, st);
+            return e;
+        }
     }
-    cudaError_t e = cudaMallocAsync(ptr, need, st);
-    if (e == cudaSuccess) *have = need;
+    *ptr = fresh;
+    *have = need;
+    return cudaSuccess;
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (kernel, DEVICE): set it once per
+// kernel instantiation and device (`devices` = bit d set when done on device d), not once per
+// process -- a second GPU would otherwise refuse the 80-120 KB launches.  Beyond 64 devices, or
+// when two host threads get here together, the attribute is simply set again (idempotent).
+template <typename Kernel>
+inline cudaError_t allow_dynamic_smem(std::atomic<unsigned long long>& devices, Kernel kern, int bytes) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool tracked = dev >= 0 && dev < 64;
+    const unsigned long long bit = tracked ? 1ULL << dev : 0ULL;
+    if (tracked && (devices.load(std::memory_order_acquire) & bit)) return cudaSuccess;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess && tracked) devices.fetch_or(bit, std::memory_order_release);
     return e;
 }
+
+// The wrap-around schedule lets a CTA wait for a piece that ANOTHER CTA of the same grid runs
+// (kernels.cuh, `dynamic == 2`): that terminates only if every CTA of the grid is resident at
+// once.  One CTA (or two) per SM always fits a whole, idle GPU, but not an MPS / green-context
+// partition with fewer SMs than cudaDevAttrMultiProcessorCount reports.  So such a grid goes out
+// as a COOPERATIVE launch: the runtime then either guarantees co-residency or refuses the launch
+// (cudaErrorCooperativeLaunchTooLarge) instead of letting it hang.  `args` are converted to the
+// kernel's exact parameter types before their addresses are taken.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_coresident(void (*kern)(KArgs...), int grid, int threads, size_t smem,
+                                     cudaStream_t st, Args&&... args) {
+    static_assert(sizeof...(KArgs) == sizeof...(Args), "one argument per kernel parameter");
+    std::tuple<std::remove_cv_t<KArgs>...> vals(std::forward<Args>(args)...);
+    return std::apply(
+        [&](auto&... v) {
+            void* argv[] = {static_cast<void*>(&v)...};
+            return cudaLaunchCooperativeKernel(reinterpret_cast<const void*>(kern), dim3((unsigned)grid),
+                                               dim3((unsigned)threads), argv, smem, st);
+        },
+        vals);
+}
+inline bool coresidency_refused(cudaError_t e) {
+    return e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorNotSupported;
+}
+// Set by a launch site whose wrap-around launch was refused and which ran the ticket queue instead
+// (safe with any number of resident CTAs: a work item only ever waits for one with a smaller
+// ticket, i.e. for a CTA that is running or done); read and cleared by the entry point, which
+// reports it in LT_STAT_LAST_MODE.  Per host thread, like the call itself.
+inline thread_local int g_wrap_refused = 0;
 
 int ensure_device(lt_tracker* tr);
 int ensure_scratch(lt_tracker* tr, int grid, cudaStream_t st);

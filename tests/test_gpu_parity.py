@@ -127,6 +127,33 @@ def test_dynamic_scheduling_is_bit_identical_to_the_plain_kernel(integrator, rat
         tr.set_option(lt.OPT_CHUNK_TURNS, 1 << 22)
 
 
+def test_wrap_around_schedule_is_a_cooperative_launch_and_survives_a_busy_gpu():
+    """The wrap-around schedule (default at the configs[1] size) makes CTAs wait on one another, so
+    it is launched cooperatively: the runtime guarantees co-residency or refuses, in which case
+    the library runs the ticket queue (LT_STAT_LAST_MODE says which).  Here the headline shape
+    runs while a second stream keeps the SMs busy with long foreign kernels: it must finish, and
+    with the same bits as on an idle GPU and as the ticket queue gives."""
+    tr, _ = both()
+    z0, d0 = wl.make_bunch(wl.CONFIGS[1])
+    turns = 3000
+    assert tr.plan_fused(z0.size, turns)["dynamic"] == 2
+    ref = gpu_track(tr, z0, d0, turns)
+    assert tr.get_stat(lt.STAT_LAST_MODE) == lt.FUSED_PERSISTENT_WRAP
+    tr.set_option(lt.OPT_FUSED_MODE, lt.FUSED_PERSISTENT_DYNAMIC)
+    queue = gpu_track(tr, z0, d0, turns)
+    assert np.array_equal(queue[0], ref[0]) and np.array_equal(queue[1], ref[1])
+    tr.set_option(lt.OPT_FUSED_MODE, lt.FUSED_AUTO)
+    side = torch.cuda.Stream()
+    a = torch.randn(8192, 8192, device="cuda")
+    with torch.cuda.stream(side):
+        for _ in range(40):                                 # ~100 ms of GEMMs holding shared memory on every SM
+            a = torch.mm(a, a).clamp_(-1.0, 1.0)
+    out = gpu_track(tr, z0, d0, turns)                      # enqueued while the GEMMs run
+    side.synchronize()
+    assert tr.get_stat(lt.STAT_LAST_MODE) in (lt.FUSED_PERSISTENT_WRAP, lt.FUSED_PERSISTENT_DYNAMIC)
+    assert np.array_equal(out[0], ref[0]) and np.array_equal(out[1], ref[1])
+
+
 def test_deterministic():
     tr, _ = both()
     z0, d0 = wl.make_bunch(wl.CONFIGS[1], n=50_000)
