@@ -10,8 +10,11 @@ register-resident (fused mode), exit store, then the bucket-membership count of 
 state.  `value` is device-timed with the bunch already in HBM; `e2e` goes through the C ABI
 with HOST buffers (lt_track_fused_host: H2D, track, count, D2H inside the timed region).
 
-Everything else the measurement contract asks for sits INSIDE `roofline` (the driver keeps
-that object whole): `per_turn` (configs[3], the HBM-bound half of the metric), `configs`
+Everything else the measurement contract asks for sits INSIDE `roofline`.  The driver's record
+keeps the SCALAR keys of that object and drops nested ones, so every leg's fraction is repeated
+as a flat key (`per_turn_frac`, `per_turn_gbs`, `cfg2_frac`, `cfg4_*_frac`, `f2_*_frac`, `f3_*`,
+`f4_*`, `f1_us_per_launch_1turn_*`, `traffic_source`; flat_summary()) and the scalars are printed
+last.  The nested legs: `per_turn` (configs[3], the HBM-bound half of the metric), `configs`
 (configs[0], [2] and the six configs[4] variants), `f1_chunk_sweep` (turns per launch 1 ..
 2^14 at a fixed total: the B200 redo of the paper's Fig. 5), `size_sweep`
 (n = 2^10 .. 2^24: the analogue of its Table 2), `next` (the
@@ -76,6 +79,8 @@ def ncu_traffic() -> dict:
                for k, v in raw.get("kernels", {}).items()}
         out.update({k + "_ncu_us": float(v["duration_us"]) for k, v in raw.get("kernels", {}).items()
                     if "duration_us" in v})
+        out.update({k + "_source": "profiles/ncu_traffic.json, captured at %s" % v.get("captured_at_commit", "?")
+                    for k, v in raw.get("kernels", {}).items()})
         return out
     except Exception:
         return {}
@@ -704,6 +709,66 @@ def bench_per_turn_sharded(cx: Ctx) -> dict:
 
 
 # ----------------------------------------------------------------------------- CUDA arm
+def flat_summary(roofline: dict, cx: Ctx) -> dict:
+    """Both halves of BASELINE.json's metric ("% of FP64 / HBM roofline") and one fraction per
+    config / sec. 8(f) row as FLAT SCALAR keys of `roofline`: the driver's record keeps the
+    scalars of that object and drops nested ones.  Values are copied from the legs above, nothing
+    is measured here; a leg that did not run (or failed) leaves its keys out."""
+    out = {"traffic_source": cx.traffic.get("fused_source")}
+
+    def leg(*path):
+        node = roofline
+        for k in path:
+            if not isinstance(node, dict) or k not in node:
+                return None
+            node = node[k]
+        return node
+
+    def put(key, value, digits=4):
+        if isinstance(value, (int, float)):
+            out[key] = round(float(value), digits)
+
+    pt = leg("per_turn")
+    if isinstance(pt, dict) and "frac" in pt:
+        put("per_turn_frac", pt["frac"])                       # algorithmic bytes / time / copy peak
+        put("per_turn_gbs", pt["achieved"], 1)
+        put("per_turn_us", 1e3 * pt["ms_per_turn"], 2)
+        put("per_turn_frac_of_8TBs", pt["frac_of_nominal_8TBs"])
+        put("per_turn_value", pt["value"], 0)
+        if pt.get("traffic"):                                  # ncu DRAM bytes (committed capture) / this run's time
+            put("per_turn_dram_frac", pt["traffic"] / (pt["ms_per_turn"] * 1e-3) / 1e9 / pt["peak"])
+        rows = leg("per_turn", "beyond_l2", "rows") or []
+        if rows:
+            put("per_turn_beyond_l2_frac_min", min(r["frac"] for r in rows))
+            put("per_turn_beyond_l2_frac_max", max(r["frac"] for r in rows))
+    for key, name in (("cfg0_frac", "configs[0]"), ("cfg2_frac", "configs[2]"),
+                      ("cfg4_ec_f64_frac", "configs[4] euler_cromer fp64"),
+                      ("cfg4_lf_f64_frac", "configs[4] leapfrog fp64"),
+                      ("cfg4_ruth4_f64_frac", "configs[4] ruth4 fp64"),
+                      ("cfg4_ec_f32_frac", "configs[4] euler_cromer fp32"),
+                      ("cfg4_lf_f32_frac", "configs[4] leapfrog fp32"),
+                      ("cfg4_ruth4_f32_frac", "configs[4] ruth4 fp32")):
+        cfgs = leg("configs") or {}
+        hit = [v for k, v in cfgs.items() if k.startswith(name) and isinstance(v, dict)]
+        if hit:
+            put(key, (hit[0].get("roofline") or {}).get("frac"))
+    for key, name in (("f2_programme_frac", "f2_programme_fused"), ("f2_ramp_frac", "f2_ramp_fused"),
+                      ("f2_programme_per_turn_frac", "f2_programme_per_turn"),
+                      ("f2_ramp_per_turn_frac", "f2_ramp_per_turn"),
+                      ("f3_fused_frac", "f3_transverse_fused"), ("f3_per_turn_frac", "f3_transverse_per_turn"),
+                      ("f4_hist_frac", "f4_slice_histogram"), ("f4_track_slices_frac", "f4_track_slices"),
+                      ("f4_track_slices_moments_frac", "f4_track_slices_with_moments")):
+        put(key, leg("next", name, "roofline", "frac"))
+    put("f4_hist_us", leg("next", "f4_slice_histogram", "us_per_call"), 2)
+    for r in leg("f1_chunk_sweep", "rows") or []:
+        if r.get("turns_per_launch") == 1:
+            tag = {"fused": "f1_us_per_launch_1turn_fused", "per_turn graph=0": "f1_us_per_launch_1turn_per_turn_stream",
+                   "per_turn graph=1": "f1_us_per_launch_1turn_per_turn_graph"}.get(r.get("kernel"))
+            if tag:
+                put(tag, r["us_per_launch"], 2)
+    return out
+
+
 def run_cuda(args) -> None:
     import numpy as np
     import torch
@@ -831,6 +896,8 @@ def run_cuda(args) -> None:
         roofline["frac_of_measured_turn_loop_ceiling"] = (
             roofline["frac"] / (max(probe["turn_flip_on_f_ilp2_w4"], probe["turn_flip_on_q_ilp1_w8"]) / 0.5))
 
+    roofline.update(flat_summary(roofline, cx))
+
     # ---- CPU oracle beside it (rank 0, N = 1 only): all cores, and one thread
     cpu_baseline = None
     if world == 1 and not args.skip_cpu:
@@ -855,8 +922,11 @@ def run_cuda(args) -> None:
                        "l2": "flushed between timed iterations (256 MB fill)",
                        "parallelism": "particles sharded, no collective (weak)"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
-            "roofline": roofline, "cpu_baseline": cpu_baseline,
-            "wall_s_timed_region": wall,
+            "cpu_baseline": cpu_baseline, "wall_s_timed_region": wall,
+            # last, and inside it the nested legs before the scalars: the tail of the line -- what a
+            # truncated log keeps -- is the compact summary (frac, per_turn_frac, cfg*_frac, f*_frac)
+            "roofline": {**{k: v for k, v in roofline.items() if isinstance(v, (dict, list))},
+                         **{k: v for k, v in roofline.items() if not isinstance(v, (dict, list))}},
         }))
     if world > 1:
         dist.destroy_process_group()
