@@ -407,7 +407,7 @@ def bench_probe(cx: Ctx, table: bool = False) -> dict:
     (16 FP64 lanes per sub-partition, 64 per SM).  table=True (`--only probe`) adds the rate of
     the turn loop for every (particles per lane, warps per sub-partition, sign-flip place): the
     planner's loop_rate table in csrc/longtrack.cu."""
-    lt = cx.lt
+    from paper_1610_05801_b200 import probe           # liblongtrack_probe.so: measurement tooling only
     out = {}
     with cx.clock() as clk:
         for name, kind, threads, chains in (("dadd", 2, 1024, 4), ("dmul", 3, 1024, 4),
@@ -418,7 +418,7 @@ def bench_probe(cx: Ctx, table: bool = False) -> dict:
                                             ("turn_flip_on_f_ilp2_w4", 11, 512, 2),
                                             ("turn_flip_on_q_ilp1_w5", 10, 640, 1),
                                             ("turn_flip_on_q_ilp1_w8", 10, 1024, 1)):
-            rate, mhz = lt.probe_pipe(kind, SMS, threads, chains, 20000 // chains)
+            rate, mhz = probe.probe_pipe(kind, SMS, threads, chains, 20000 // chains)
             out[name] = round(rate, 4)
             out["sm_mhz_under_fp64_load"] = round(mhz)
         if table:
@@ -426,7 +426,7 @@ def bench_probe(cx: Ctx, table: bool = False) -> dict:
             for kind, name in ((11, "flip_on_f"), (10, "flip_on_q"), (12, "no_flip")):
                 for chains in (1, 2, 4):
                     tab["%s ilp%d W=1..8" % (name, chains)] = [
-                        round(lt.probe_pipe(kind, SMS, 128 * w, chains, 8000 // chains)[0], 4)
+                        round(probe.probe_pipe(kind, SMS, 128 * w, chains, 8000 // chains)[0], 4)
                         for w in range(1, 9)]
             out["turn_loop_table"] = tab
     out["unit"] = "FP64 warp-instr/cycle/sub-partition (nominal peak 0.5)"

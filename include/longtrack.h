@@ -35,8 +35,8 @@
  *     required; 16-byte alignment enables the vector path (otherwise a scalar path runs).
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device
  *     calls only ENQUEUE work on that stream and return; nothing synchronises the device.
- *     Results are valid once the caller has synchronised the stream.  The *_host calls and the
- *     lt_probe_* calls are the exception: they run to completion before they return.
+ *     Results are valid once the caller has synchronised the stream.  The *_host calls are the
+ *     exception: they run to completion before they return.
  *     The tracker's scratch is grown STREAM-ORDERED on the caller's stream (cudaMallocAsync /
  *     cudaFreeAsync): a call that needs more scratch than any before it (a larger n, a longer
  *     table) allocates without a device synchronisation, but it must not be issued while the
@@ -402,24 +402,6 @@ int lt_plan_fused(const lt_tracker *tr, size_t n, unsigned long long turns, int 
                   long long plan[7]);
 int lt_item_schedule(unsigned int turns, unsigned int item_turns, int taper, unsigned int c,
                      unsigned int *nchunks, unsigned int *start, unsigned int *len);
-
-/* -- roofline probes (measurement only, not on the hot path) ------------------------------
- * Runs a dependent-chain DFMA kernel (`chains` independent chains per thread, `iters` FMAs
- * per chain) and returns achieved FP64 lane-instructions per second in *rate. Synchronises. */
-int lt_probe_fp64(int blocks, int threads, int chains, long long iters, double *rate_host,
-                  double *ms_host);
-/* What the FP64 pipe of the device at hand issues, counted with clock64 (so independent of the
- * clock): `threads` (multiple of 32, <= 1024) threads in each of `blocks` CTAs (one CTA per SM:
- * pass the SM count) run `chains` (1, 2, 4) independent dependent chains of 8 * iters steps of
- *   kind 0  DFMA with three register operands      kind 1  DFMA, two registers + a uniform operand
- *   kind 2  DADD                                   kind 3  DMUL
- *   kind 10 / 11 / 12  the 13-instruction leap-frog turn of the fused kernel
- *                      with the sign flip on the polynomial / on the argument / left out.
- * *instr_per_cycle_host = FP64 warp-instructions per cycle and SM sub-partition (the pipe's
- * nominal peak is 0.5: 16 lanes per sub-partition); *sm_clock_mhz_host (may be NULL) = SM clock
- * during the probe, from clock64 against the nanosecond global timer.  Synchronises. */
-int lt_probe_pipe(int kind, int blocks, int threads, int chains, long long iters,
-                  double *instr_per_cycle_host, double *sm_clock_mhz_host);
 
 #ifdef __cplusplus
 }

@@ -1,4 +1,4 @@
-"""Builds liblongtrack.so for sm_100a with nvcc (in-tree, next to this file).
+"""Builds liblongtrack.so and liblongtrack_probe.so for sm_100a with nvcc (in-tree, next to this file).
 
     python -m paper_1610_05801_b200.build [--force]
 
@@ -18,9 +18,16 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblongtrack.so")
 SOURCES = [os.path.join(CSRC, "longtrack.cu"), os.path.join(CSRC, "longtrack_next.cu"),
            os.path.join(CSRC, "longtrack_ramp.cu"), os.path.join(CSRC, "longtrack_static.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "kernels_next.cuh"), os.path.join(CSRC, "kernels_ramp.cuh"), os.path.join(CSRC, "kernels_probe.cuh"),
+DEPS = SOURCES + [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "kernels_next.cuh"), os.path.join(CSRC, "kernels_ramp.cuh"),
                   os.path.join(CSRC, "tracker.hpp"), os.path.join(CSRC, "sinpi_coeffs.h"),
                   os.path.join(ROOT, "include", "longtrack.h")]
+
+# measurement tooling (FP64-pipe probes), its own library: liblongtrack.so exports the tracking calls only
+PROBE_LIB = os.path.join(HERE, "liblongtrack_probe.so")
+PROBE_SOURCES = [os.path.join(CSRC, "longtrack_probe.cu")]
+PROBE_DEPS = PROBE_SOURCES + [os.path.join(CSRC, "kernels.cuh"), os.path.join(CSRC, "kernels_probe.cuh"),
+                              os.path.join(CSRC, "sinpi_coeffs.h"), os.path.join(ROOT, "include", "longtrack.h"),
+                              os.path.join(ROOT, "include", "longtrack_probe.h")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "--threads", "2"]
@@ -33,25 +40,31 @@ def nvcc() -> str:
     return exe
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    newest = max(os.path.getmtime(p) for p in DEPS)
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
-        return LIB
-    # nvcc/ld write their output in place: link to a private name and rename it onto LIB, so that
-    # another process (the non-zero ranks of a torchrun launch, wait_until_built below) can never
-    # dlopen a half-written library -- os.replace is atomic within one directory
-    tmp = "%s.tmp.%d" % (LIB, os.getpid())
-    cmd = [nvcc(), *NVCC_FLAGS, "-o", tmp, *SOURCES]
+def _build_one(lib: str, sources: list, deps: list, force: bool, verbose: bool) -> str:
+    newest = max(os.path.getmtime(p) for p in deps)
+    if not force and os.path.exists(lib) and os.path.getmtime(lib) >= newest:
+        return lib
+    # nvcc/ld write their output in place: link to a private name and rename it onto the library, so
+    # that another process (the non-zero ranks of a torchrun launch, wait_until_built below) can never
+    # dlopen a half-written file -- os.replace is atomic within one directory
+    tmp = "%s.tmp.%d" % (lib, os.getpid())
+    cmd = [nvcc(), *NVCC_FLAGS, "-o", tmp, *sources]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd))
     try:
         subprocess.run(cmd, check=True, cwd=HERE)
-        os.replace(tmp, LIB)
+        os.replace(tmp, lib)
     finally:
         if os.path.exists(tmp):
             os.remove(tmp)
-    return LIB
+    return lib
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """liblongtrack.so (the product) and liblongtrack_probe.so (bench.py's FP64-pipe probes)."""
+    _build_one(PROBE_LIB, PROBE_SOURCES, PROBE_DEPS, force, verbose)
+    return _build_one(LIB, SOURCES, DEPS, force, verbose)       # last: wait_until_built watches this one
 
 
 def wait_until_built(timeout_s: float = 900.0) -> str:
@@ -59,7 +72,9 @@ def wait_until_built(timeout_s: float = 900.0) -> str:
     import time
     t0 = time.time()
     newest = max(os.path.getmtime(p) for p in DEPS)
-    while not (os.path.exists(LIB) and os.path.getmtime(LIB) >= newest):
+    newest_probe = max(os.path.getmtime(p) for p in PROBE_DEPS)
+    while not (os.path.exists(LIB) and os.path.getmtime(LIB) >= newest and
+               os.path.exists(PROBE_LIB) and os.path.getmtime(PROBE_LIB) >= newest_probe):
         if time.time() - t0 > timeout_s:
             raise RuntimeError("liblongtrack.so was not built within %.0f s" % timeout_s)
         time.sleep(0.5)

@@ -93,10 +93,6 @@ def _load():
         "lt_moments_now_static": (c_int, [vp, vp, vp, sz, vp, vp, vp]),
         "lt_moments_from_sums": (c_int, [vp, sz, vp]),
         "lt_track_fused_host": (c_int, [vp, vp, vp, sz, ull, POINTER(ull)]),
-        "lt_probe_fp64": (c_int, [c_int, c_int, c_int, c_longlong, POINTER(c_double),
-                                  POINTER(c_double)]),
-        "lt_probe_pipe": (c_int, [c_int, c_int, c_int, c_int, c_longlong, POINTER(c_double),
-                                  POINTER(c_double)]),
         "lt_plan_fused": (c_int, [vp, sz, ull, c_int, c_int, POINTER(c_longlong)]),
         "lt_item_schedule": (c_int, [ctypes.c_uint, ctypes.c_uint, c_int, ctypes.c_uint,
                                      POINTER(ctypes.c_uint), POINTER(ctypes.c_uint),
@@ -298,23 +294,6 @@ def moments_from_sums(sums: np.ndarray) -> np.ndarray:
     if rc != OK:
         raise LongtrackError(rc)
     return out
-
-
-def probe_fp64(blocks: int, threads: int, chains: int, iters: int):
-    rate, ms = c_double(), c_double()
-    rc = _lib.lt_probe_fp64(blocks, threads, chains, iters, byref(rate), byref(ms))
-    if rc != OK:
-        raise LongtrackError(rc)
-    return rate.value, ms.value
-
-
-def probe_pipe(kind: int, blocks: int, threads: int, chains: int, iters: int):
-    """Returns (FP64 warp-instructions per cycle per sub-partition, SM clock in MHz)."""
-    rate, mhz = c_double(), c_double()
-    rc = _lib.lt_probe_pipe(kind, blocks, threads, chains, iters, byref(rate), byref(mhz))
-    if rc != OK:
-        raise LongtrackError(rc)
-    return rate.value, mhz.value
 
 
 def item_schedule(turns: int, item_turns: int, taper: bool = True):

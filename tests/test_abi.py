@@ -18,8 +18,8 @@ def lt():
     return longtrack
 
 
-def declared_functions():
-    src = open(os.path.join(ROOT, "include", "longtrack.h")).read()
+def declared_functions(header="longtrack.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(lt_[a-z0-9_]+)\s*\(", src)))
 
@@ -32,6 +32,21 @@ def test_every_declared_symbol_is_exported_and_bound(lt):
     for n in names:
         assert hasattr(lib, n), "missing export " + n
     assert sorted(lt.EXPORTS) == names      # the binding covers exactly the header
+
+
+def test_probe_library_is_separate_and_complete(lt):
+    """The FP64-pipe probes are bench tooling: their own header and library; liblongtrack.so
+    exports the tracking calls only."""
+    import ctypes
+    from paper_1610_05801_b200 import probe
+    names = declared_functions("longtrack_probe.h")
+    assert names == ["lt_probe_fp64", "lt_probe_pipe"] == sorted(probe.EXPORTS)
+    plib = ctypes.CDLL(probe.LIB_PATH)
+    main = ctypes.CDLL(lt.LIB_PATH)
+    for n in names:
+        assert hasattr(plib, n), "missing export " + n
+        assert not hasattr(main, n), n + " is still exported by liblongtrack.so"
+    assert not any(n.startswith("lt_probe") for n in declared_functions())
 
 
 def test_version_and_strerror(lt):
